@@ -1,0 +1,136 @@
+/*
+ * fdas.h -- C ABI of libfdas.so: the FDAS matched-filter hot path on one B200 (sm_100a).
+ *
+ * What the library computes (arXiv:1711.10855; P:NN = line NN of the paper text, PAPER.md):
+ *
+ *   eq.(2), P:21-23   A'_{r0} = sum_k A_k conj(H_{r0-k})   "correlating the m bins around bin r0 with
+ *                     the predicted, normalized, Fourier response H", for every acceleration trial z,
+ *   P:31 (section 2)  evaluated by overlap-and-save: the spectrum is cut into segments of length L,
+ *                     each is Fourier transformed on chip (eq.(3)), multiplied by the
+ *                     transformed template of every z, inverse transformed, trimmed of its aliased
+ *                     part and merged "in such a way as to produce the linear convolution",
+ *   BASELINE.json     and written as the float32 power plane P[z][r0] = |A'_{r0}|^2.
+ *
+ * With the template of trial z given as m taps h_z[j], tap j <-> offset d = j - m/2 (DESIGN.md,
+ * readings 1, 6, 7):
+ *
+ *   P[b][i][r0] = | sum_{j=0}^{m-1} A[b][r0 + m/2 - j] * conj(h_i[j]) |^2 ,   A[b][k] := 0 for k outside [0, n_f)
+ *
+ * for batch item b < n_batch, template row i < n_z (row i <-> z = -z_max + i*z_step), column r0 < n_f.
+ * All arithmetic is IEEE float32 (FMA contraction allowed); the result equals the definition up to
+ * rounding.  There is no CPU fallback: every entry point that needs the GPU fails with FDAS_ERR_CUDA
+ * if none is usable.
+ *
+ * Conventions: "HOST" / "DEVICE" say where a pointer must live.  Complex data are interleaved
+ * (re, im) float32 pairs.  No exception crosses this boundary; no global state; a plan may be used
+ * from several host threads as long as calls on the same plan are not concurrent.
+ */
+#ifndef FDAS_H
+#define FDAS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdas_plan fdas_plan; /* opaque; owned by the library between create and destroy */
+
+typedef enum {
+    FDAS_OK = 0,
+    FDAS_ERR_INVALID_ARG = 1,  /* NULL pointer, bad size, misaligned buffer */
+    FDAS_ERR_UNSUPPORTED = 2,  /* segment_len not in {512, 1024, 2048, 4096, 8192} */
+    FDAS_ERR_ALLOC = 3,        /* host or device allocation failed */
+    FDAS_ERR_NO_TEMPLATES = 4, /* fdas_convolve before fdas_set_templates */
+    FDAS_ERR_CUDA = 5          /* a CUDA runtime call failed; see fdas_plan_last_cuda_error */
+} fdas_status;
+
+/*
+ * Create a plan for spectra of n_f bins, trials z = -z_max, -z_max+z_step, ..., +z_max
+ * (n_z = 2*z_max/z_step + 1), templates of template_width = m taps and overlap-and-save segments of
+ * segment_len = L points (argument list from BASELINE.json north_star).  The plan keeps
+ * S = L - m outputs per segment (any step <= L-m+1 gives the same linear convolution, P:31;
+ * DESIGN.md reading 8) and n_seg = ceil(n_f / S) segments per spectrum.  Batch count starts at 1.
+ *
+ *   out            HOST, receives the plan; untouched on error
+ *   n_f            >= 1
+ *   z_max, z_step  z_max >= 0, z_step >= 1, z_max % z_step == 0
+ *   template_width even, >= 2, <= segment_len / 2
+ *   segment_len    512, 1024, 2048, 4096 or 8192 (else FDAS_ERR_UNSUPPORTED)
+ *
+ * Allocates plan-owned device memory on the current CUDA device: the transformed template bank
+ * (n_z * L complex64) and a twiddle table (L complex64, eq.(3)).
+ */
+fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step,
+                             int template_width, int segment_len);
+
+/* Number of independent spectra one fdas_convolve call processes (BASELINE.json config 5:
+ * "64 independent spectra ... computed in one fdas_convolve call").  n_batch >= 1.  Templates are
+ * shared by all batch items.  Cheap; may be called between convolves. */
+fdas_status fdas_plan_set_batch(fdas_plan *plan, int n_batch);
+
+/*
+ * Give the plan its template bank ("predicted, normalized, Fourier response H").
+ *   h_templates   HOST, float32 [n_z][m][2] (re, im); row i <-> z = -z_max + i*z_step; tap j <-> offset
+ *                 j - m/2.  Copied during the call; the caller may free it afterwards.
+ * The library conjugates the taps (eq.(2): conj(H)), zero-pads to L, scales by 1/L (the inverse
+ * transform's factor, reading 9), transforms them with its own FFT kernel and stores the
+ * spectra in the register order the convolution kernel reads.  Synchronous: returns after the
+ * device work has finished.  May be called again to replace the bank.
+ */
+fdas_status fdas_set_templates(fdas_plan *plan, const float *h_templates);
+
+/*
+ * Enqueue the hot path on cuda_stream: for every batch item, segment and trial z -- segment load,
+ * forward FFT (once per segment), pointwise multiply, inverse FFT, trim, |.|^2, power-plane write.
+ *   d_spectrum    DEVICE, complex64 [n_batch][n_f], read only, 8-byte aligned
+ *   d_power       DEVICE, float32 [n_batch][n_z][n_f], written completely, 4-byte aligned (128-byte
+ *                 alignment and n_f % 32 == 0 give fully coalesced line writes)
+ *   cuda_stream   a cudaStream_t passed as void* (NULL = the legacy default stream)
+ * Asynchronous: only launches; never synchronises, allocates or copies.  The buffers must stay
+ * valid until the stream has run the work.  Output is bitwise reproducible (no atomics).
+ * Errors: INVALID_ARG (NULL / misaligned pointers), NO_TEMPLATES, CUDA (launch failure).
+ */
+fdas_status fdas_convolve(fdas_plan *plan, const void *d_spectrum, float *d_power, void *cuda_stream);
+
+/*
+ * Convenience for callers whose data live in HOST memory (bench.py's "e2e" leg): copies
+ * h_spectrum to a plan-owned device buffer, runs fdas_convolve, copies the power plane back to
+ * h_power, and synchronises the stream.  Buffers are allocated on first use and kept by the plan.
+ *   h_spectrum    HOST (pinned memory gives asynchronous copies), complex64 [n_batch][n_f]
+ *   h_power       HOST, float32 [n_batch][n_z][n_f]
+ */
+fdas_status fdas_convolve_host(fdas_plan *plan, const void *h_spectrum, float *h_power, void *cuda_stream);
+
+/* Free the plan and everything it owns.  NULL is accepted. */
+fdas_status fdas_plan_destroy(fdas_plan *plan);
+
+/* Plan geometry (0 / -1 on NULL). */
+int fdas_plan_nz(const fdas_plan *plan);            /* n_z */
+int fdas_plan_step(const fdas_plan *plan);          /* S = outputs kept per segment */
+int64_t fdas_plan_nseg(const fdas_plan *plan);      /* segments per spectrum */
+int fdas_plan_batch(const fdas_plan *plan);         /* n_batch */
+
+/* Number of kernel launches the last fdas_convolve on this plan made (bench.py "gpu_launches"). */
+int fdas_plan_last_launch_count(const fdas_plan *plan);
+
+/* cudaError_t of the last failing CUDA call on this plan (0 if none), and its text. */
+int fdas_plan_last_cuda_error(const fdas_plan *plan);
+const char *fdas_status_string(fdas_status s);
+
+/*
+ * Debug / test entry: forward FFT (eq.(3)) of n_seg contiguous length-L segments with the
+ * same device code the hot path uses, returned in NATURAL frequency order.
+ *   d_in, d_out   DEVICE, complex64 [n_seg][L]; must not overlap
+ *   inverse       0: eq.(3);  1: the unnormalised inverse (conjugate twiddles)
+ * Synchronous.  Used by tests/ to check the segment FFT against the oracle's brute-force DFT.
+ */
+fdas_status fdas_debug_fft(int segment_len, int64_t n_seg, const void *d_in, void *d_out, int inverse);
+
+/* Library build info: e.g. "libfdas sm_100a <date>".  Never NULL. */
+const char *fdas_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDAS_H */

@@ -1,0 +1,153 @@
+"""Thin ctypes binding over libfdas.so (include/fdas.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used by callers for device
+memory and streams; this module only needs `.data_ptr()` / `.cuda_stream` from them.  If libfdas.so
+is missing this module raises on first use -- there is no fallback.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libfdas.so")
+
+FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_UNSUPPORTED, FDAS_ERR_ALLOC, FDAS_ERR_NO_TEMPLATES, FDAS_ERR_CUDA = range(6)
+
+# every symbol include/fdas.h declares: name -> (restype, argtypes)
+_vp, _i64, _int = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+SYMBOLS = {
+    "fdas_plan_create": (_int, [ctypes.POINTER(_vp), _i64, _int, _int, _int, _int]),
+    "fdas_plan_set_batch": (_int, [_vp, _int]),
+    "fdas_set_templates": (_int, [_vp, _vp]),
+    "fdas_convolve": (_int, [_vp, _vp, _vp, _vp]),
+    "fdas_convolve_host": (_int, [_vp, _vp, _vp, _vp]),
+    "fdas_plan_destroy": (_int, [_vp]),
+    "fdas_plan_nz": (_int, [_vp]),
+    "fdas_plan_step": (_int, [_vp]),
+    "fdas_plan_nseg": (_i64, [_vp]),
+    "fdas_plan_batch": (_int, [_vp]),
+    "fdas_plan_last_launch_count": (_int, [_vp]),
+    "fdas_plan_last_cuda_error": (_int, [_vp]),
+    "fdas_status_string": (ctypes.c_char_p, [_int]),
+    "fdas_debug_fft": (_int, [_int, _i64, _vp, _vp, _int]),
+    "fdas_version": (ctypes.c_char_p, []),
+}
+
+_LIB = None
+
+
+class FdasError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        super().__init__(f"{where}: {status_string(status)}")
+
+
+def lib():
+    """Load libfdas.so (never builds it; see paper_1711_10855_b200.build)."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1711_10855_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _LIB = L
+    return _LIB
+
+
+def status_string(s) -> str:
+    return lib().fdas_status_string(int(s)).decode()
+
+
+def version() -> str:
+    return lib().fdas_version().decode()
+
+
+def _check(s, where):
+    if s != FDAS_OK:
+        raise FdasError(s, where)
+
+
+def _ptr(x):
+    """Device/host address of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    raise TypeError(type(x))
+
+
+def _stream(s):
+    if s is None:
+        return None
+    if isinstance(s, int):
+        return s
+    return s.cuda_stream  # torch.cuda.Stream
+
+
+class Plan:
+    """fdas_plan_create ... fdas_plan_destroy as a Python object (same names, same arguments)."""
+
+    def __init__(self, n_f, z_max, z_step, template_width, segment_len, n_batch=1):
+        self._h = _vp()
+        _check(lib().fdas_plan_create(ctypes.byref(self._h), int(n_f), int(z_max), int(z_step),
+                                      int(template_width), int(segment_len)), "fdas_plan_create")
+        self.n_f, self.m, self.L = int(n_f), int(template_width), int(segment_len)
+        if n_batch != 1:
+            self.set_batch(n_batch)
+
+    # geometry
+    @property
+    def n_z(self): return lib().fdas_plan_nz(self._h)
+    @property
+    def step(self): return lib().fdas_plan_step(self._h)
+    @property
+    def n_seg(self): return lib().fdas_plan_nseg(self._h)
+    @property
+    def n_batch(self): return lib().fdas_plan_batch(self._h)
+    @property
+    def last_launch_count(self): return lib().fdas_plan_last_launch_count(self._h)
+    @property
+    def last_cuda_error(self): return lib().fdas_plan_last_cuda_error(self._h)
+
+    def set_batch(self, n_batch):
+        _check(lib().fdas_plan_set_batch(self._h, int(n_batch)), "fdas_plan_set_batch")
+
+    def set_templates(self, h_templates):
+        """h_templates: complex64 [n_z][m] numpy array (HOST)."""
+        h = np.ascontiguousarray(h_templates, dtype=np.complex64)
+        if h.shape != (self.n_z, self.m):
+            raise ValueError(f"templates must be [{self.n_z}][{self.m}], got {h.shape}")
+        _check(lib().fdas_set_templates(self._h, h.ctypes.data), "fdas_set_templates")
+
+    def convolve(self, d_spectrum, d_power, stream=None):
+        """d_spectrum: DEVICE complex64 [n_batch][n_f]; d_power: DEVICE float32 [n_batch][n_z][n_f]."""
+        _check(lib().fdas_convolve(self._h, _ptr(d_spectrum), _ptr(d_power), _stream(stream)), "fdas_convolve")
+
+    def convolve_host(self, h_spectrum, h_power, stream=None):
+        """HOST buffers (pinned torch tensors or numpy arrays); copies are inside the call."""
+        _check(lib().fdas_convolve_host(self._h, _ptr(h_spectrum), _ptr(h_power), _stream(stream)),
+               "fdas_convolve_host")
+
+    def destroy(self):
+        if self._h:
+            lib().fdas_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def debug_fft(segment_len, n_seg, d_in, d_out, inverse=False):
+    _check(lib().fdas_debug_fft(int(segment_len), int(n_seg), _ptr(d_in), _ptr(d_out), int(bool(inverse))),
+           "fdas_debug_fft")

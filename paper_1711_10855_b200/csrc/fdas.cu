@@ -1,0 +1,491 @@
+// fdas.cu -- libfdas.so: kernels and C ABI of the FDAS matched-filter hot path (include/fdas.h).
+//
+// arXiv:1711.10855 (P:NN = PAPER.md line NN): eq.(2) P:23 evaluated by overlap-and-save with
+// an on-chip FFT (eq.(3)) that is called once forward per segment and once inverse
+// per matched filter ("called for every matched filter").  One CTA owns one segment: the
+// forward-transformed segment stays in REGISTERS across all n_z templates, so the spectrum is read
+// from HBM once per segment and the only HBM stream of the z loop is the coalesced power-plane write.
+//
+// Built for sm_100a only.  No cuFFT, no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "../../include/fdas.h"
+#include "fft_device.cuh"
+
+namespace fdas {
+
+struct ConvParams {
+    const float2 *__restrict__ spectrum; // [n_batch][n_f]
+    float *__restrict__ power;           // [n_batch][n_z][n_f]
+    const float4 *__restrict__ gperm;    // [n_z][E/2][NT] : template spectra in register order
+    const float2 *__restrict__ tw;       // [L] : w_L^j
+    int64_t n_f;
+    int64_t n_seg;
+    int n_z;
+    int m;
+    int S;
+};
+
+// Inverse-pass twiddles kept in registers across the z loop (they do not depend on z): the
+// paper's "reuse already calculated twiddle factors" taken to its limit.
+template <class C> struct InvTw { float2 w[C::P - 1][C::E]; };
+
+template <class C, int I> __device__ __forceinline__ void load_inv_tw(InvTw<C> &T, const float2 *__restrict__ tw, int t)
+{
+    if constexpr (I < C::P - 1) {
+        const int u = tw_unit<C, I>(t);
+#pragma unroll
+        for (int d = 1; d < C::R(I); ++d) T.w[I][d] = __ldg(tw + d * u);
+        load_inv_tw<C, I + 1>(T, tw, t);
+    }
+}
+
+// Inverse passes: v enters in layout I+1 with its butterflies done; exchange to layout I, apply the
+// conjugate twiddles, butterfly; recurse down to pass 0.  One barrier per exchange; the two
+// buffers alternate so a buffer is rewritten only after a later barrier.
+template <class C, int I> __device__ __forceinline__ void inv_down(float2 *v, float2 *buf0, float2 *buf1,
+                                                                    const InvTw<C> &T, const int *bases)
+{
+    constexpr int R = C::R(I), B = C::E / R;
+    float2 *buf = (I & 1) ? buf1 : buf0;
+    sm_write<C, I + 1>(buf, bases[I + 1], v);
+    __syncthreads();
+    sm_read<C, I>(buf, bases[I], v);
+#pragma unroll
+    for (int d = 1; d < R; ++d)
+#pragma unroll
+        for (int b = 0; b < B; ++b) v[b * R + d] = cmulc(v[b * R + d], T.w[I][d]);
+    butterflies<C, I, true>(v);
+    if constexpr (I > 0) inv_down<C, I - 1>(v, buf0, buf1, T, bases);
+}
+
+template <class C, int I> __device__ __forceinline__ void fill_bases(int *bases, int t)
+{
+    bases[I] = lay_base<C, I>(t);
+    if constexpr (I + 1 < C::P) fill_bases<C, I + 1>(bases, t);
+}
+
+// -------------------------------------------------------------------------------------------
+// Hot kernel: steps a1..a6 of DESIGN.md for one (batch item, segment), all z.
+// -------------------------------------------------------------------------------------------
+template <int L, int MINB>
+__global__ void __launch_bounds__(Cfg<L>::NT, MINB) fdas_convolve_kernel(const ConvParams p)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, NT = C::NT;
+    extern __shared__ float2 smem[];
+    float2 *buf0 = smem, *buf1 = smem + C::SMEM_ELEMS;
+    const int t = threadIdx.x;
+    const int64_t seg = blockIdx.x % p.n_seg;
+    const int64_t bi = blockIdx.x / p.n_seg;
+
+    // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
+    float2 v[E];
+    {
+        const float2 *__restrict__ A = p.spectrum + bi * p.n_f;
+        const int64_t base = seg * p.S - p.m / 2;
+#pragma unroll
+        for (int d = 0; d < E; ++d) {
+            const int64_t k = base + d * NT + t;
+            v[d] = (k >= 0 && k < p.n_f) ? __ldg(A + k) : make_float2(0.f, 0.f);
+        }
+    }
+    // a2: forward FFT, once per segment (eq.(3))
+    fwd_from<C, 0>(v, buf0, buf1, p.tw, t);
+    float2 X[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) X[e] = v[e];
+    __syncthreads();
+
+    int bases[C::P];
+    fill_bases<C, 0>(bases, t);
+    InvTw<C> T;
+    load_inv_tw<C, 0>(T, p.tw, t);
+
+    // output geometry: register d of layout 0 holds y[d*NT + t]; kept if >= m; column = seg*S + p - m
+    const int64_t col0 = seg * p.S - p.m + t;                 // column of y[t]
+    float *__restrict__ prow = p.power + bi * p.n_z * p.n_f;  // row 0 of this batch item
+    const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
+    const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
+    const int d0 = p.m / NT;
+
+    const float4 *__restrict__ gp = p.gperm + t;
+    float4 g[E / 2];
+#pragma unroll
+    for (int q = 0; q < E / 2; ++q) g[q] = __ldg(gp + q * NT);
+
+    for (int z = 0; z < p.n_z; ++z) {
+        // a3: pointwise multiply by the transformed template ("convolution in the Fourier domain")
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) {
+            v[2 * q] = cmul(X[2 * q], make_float2(g[q].x, g[q].y));
+            v[2 * q + 1] = cmul(X[2 * q + 1], make_float2(g[q].z, g[q].w));
+        }
+        // prefetch the next template spectrum (L2 resident) while this one is transformed
+        if (z + 1 < p.n_z) {
+            gp += (E / 2) * NT;
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) g[q] = __ldg(gp + q * NT);
+        }
+        // a4: inverse FFT
+        butterflies<C, C::P - 1, true>(v);
+        inv_down<C, C::P - 2>(v, buf0, buf1, T, bases);
+        if constexpr ((C::P - 1) & 1) __syncthreads(); // odd number of exchanges: protect buffer reuse
+        // a5 + a6: trim, power, coalesced store
+        float *__restrict__ out = prow + (int64_t)z * p.n_f + col0;
+        if (fast) {
+#pragma unroll
+            for (int d = 0; d < E; ++d) {
+                if (d >= 4 || d >= d0) __stcs(out + d * NT, v[d].x * v[d].x + v[d].y * v[d].y);
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < E; ++d) {
+                const int pidx = d * NT + t;
+                const int64_t col = col0 + d * NT;
+                if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = v[d].x * v[d].x + v[d].y * v[d].y;
+            }
+        }
+    }
+}
+
+// -------------------------------------------------------------------------------------------
+// Template preparation (off the hot path): G_z = DFT_L(pad(conj h_z)) / L in register order.
+// -------------------------------------------------------------------------------------------
+template <int L>
+__global__ void __launch_bounds__(Cfg<L>::NT) fdas_template_fft_kernel(const float2 *__restrict__ h, int m,
+                                                                       const float2 *__restrict__ tw,
+                                                                       float4 *__restrict__ gperm)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, NT = C::NT;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x;
+    const int z = blockIdx.x;
+    const float scale = 1.0f / (float)L;
+    float2 v[E];
+#pragma unroll
+    for (int d = 0; d < E; ++d) {
+        const int j = d * NT + t;
+        float2 a = make_float2(0.f, 0.f);
+        if (j < m) { a = h[(size_t)z * m + j]; a.x *= scale; a.y *= -scale; } // conj(h) / L
+        v[d] = a;
+    }
+    fwd_from<C, 0>(v, smem, smem + C::SMEM_ELEMS, tw, t);
+    float4 *g = gperm + (size_t)z * (E / 2) * NT + t;
+#pragma unroll
+    for (int q = 0; q < E / 2; ++q) g[q * NT] = make_float4(v[2 * q].x, v[2 * q].y, v[2 * q + 1].x, v[2 * q + 1].y);
+}
+
+// -------------------------------------------------------------------------------------------
+// Debug FFT: natural order in, natural order out, either direction (tests only).
+// -------------------------------------------------------------------------------------------
+template <int L>
+__global__ void __launch_bounds__(Cfg<L>::NT) fdas_debug_fft_kernel(const float2 *__restrict__ in, float2 *__restrict__ out,
+                                                                    const float2 *__restrict__ tw, int inverse)
+{
+    using C = Cfg<L>;
+    constexpr int E = C::E, NT = C::NT, RL = C::R(C::P - 1), BL = E / RL;
+    extern __shared__ float2 smem[];
+    float2 *buf0 = smem, *buf1 = smem + C::SMEM_ELEMS;
+    const int t = threadIdx.x;
+    const float2 *x = in + (size_t)blockIdx.x * L;
+    float2 *y = out + (size_t)blockIdx.x * L;
+    float2 v[E];
+    if (!inverse) {
+#pragma unroll
+        for (int d = 0; d < E; ++d) v[d] = x[d * NT + t];
+        __syncthreads();
+        fwd_from<C, 0>(v, buf0, buf1, tw, t);
+#pragma unroll
+        for (int b = 0; b < BL; ++b)
+#pragma unroll
+            for (int d = 0; d < RL; ++d) y[nat_freq<C>(t, b, d)] = v[b * RL + d];
+    } else {
+#pragma unroll
+        for (int b = 0; b < BL; ++b)
+#pragma unroll
+            for (int d = 0; d < RL; ++d) v[b * RL + d] = x[nat_freq<C>(t, b, d)];
+        __syncthreads();
+        int bases[C::P];
+        fill_bases<C, 0>(bases, t);
+        InvTw<C> T;
+        load_inv_tw<C, 0>(T, tw, t);
+        butterflies<C, C::P - 1, true>(v);
+        inv_down<C, C::P - 2>(v, buf0, buf1, T, bases);
+#pragma unroll
+        for (int d = 0; d < E; ++d) y[d * NT + t] = v[d];
+    }
+}
+
+} // namespace fdas
+
+// =============================================================================================
+// host side
+// =============================================================================================
+using namespace fdas;
+
+struct fdas_plan {
+    int64_t n_f;
+    int z_max, z_step, n_z, m, L, S;
+    int64_t n_seg;
+    int n_batch;
+    float4 *d_gperm;   // n_z * L complex64
+    float2 *d_tw;      // L complex64
+    bool has_templates;
+    int last_cuda_error;
+    int last_launches;
+    // buffers of fdas_convolve_host
+    void *d_host_spec;
+    float *d_host_power;
+    size_t host_spec_bytes, host_power_bytes;
+};
+
+namespace {
+
+bool supported_L(int L) { return L == 512 || L == 1024 || L == 2048 || L == 4096 || L == 8192; }
+
+fdas_status cuda_fail(fdas_plan *p, cudaError_t e)
+{
+    if (p) p->last_cuda_error = (int)e;
+    (void)cudaGetLastError();
+    return FDAS_ERR_CUDA;
+}
+
+// w_L^j = exp(-i 2 pi j / L), computed in double, rounded once (eq.(3), "twiddle factors")
+cudaError_t upload_twiddles(int L, float2 **d_tw)
+{
+    float2 *h = (float2 *)malloc(sizeof(float2) * (size_t)L);
+    if (!h) return cudaErrorMemoryAllocation;
+    for (int j = 0; j < L; ++j) {
+        // exact octant symmetry is not needed at the tolerance; plain double evaluation
+        const double a = -2.0 * M_PI * (double)j / (double)L;
+        h[j].x = (float)cos(a);
+        h[j].y = (float)sin(a);
+    }
+    cudaError_t e = cudaMalloc((void **)d_tw, sizeof(float2) * (size_t)L);
+    if (e == cudaSuccess) e = cudaMemcpy(*d_tw, h, sizeof(float2) * (size_t)L, cudaMemcpyHostToDevice);
+    free(h);
+    return e;
+}
+
+template <int L> size_t smem_bytes() { return 2 * sizeof(float2) * (size_t)Cfg<L>::SMEM_ELEMS; }
+
+template <int L, int MINB> cudaError_t launch_convolve(const ConvParams &cp, int n_batch, cudaStream_t st)
+{
+    auto kern = fdas_convolve_kernel<L, MINB>;
+    static bool attr_done = false; // per instantiation; benign race (idempotent)
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<L>());
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int64_t blocks = cp.n_seg * n_batch;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    kern<<<(unsigned)blocks, Cfg<L>::NT, smem_bytes<L>(), st>>>(cp);
+    return cudaGetLastError();
+}
+
+template <int L> cudaError_t launch_template_fft(const float2 *d_h, int m, int n_z, const float2 *d_tw, float4 *d_g)
+{
+    auto kern = fdas_template_fft_kernel<L>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<L>());
+    if (e != cudaSuccess) return e;
+    kern<<<n_z, Cfg<L>::NT, smem_bytes<L>()>>>(d_h, m, d_tw, d_g);
+    return cudaGetLastError();
+}
+
+template <int L> cudaError_t launch_debug_fft(int64_t n_seg, const float2 *in, float2 *out, const float2 *d_tw, int inverse)
+{
+    auto kern = fdas_debug_fft_kernel<L>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<L>());
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)n_seg, Cfg<L>::NT, smem_bytes<L>()>>>(in, out, d_tw, inverse);
+    return cudaGetLastError();
+}
+
+#define FDAS_DISPATCH_L(L, EXPR)                  \
+    switch (L) {                                  \
+    case 512: { constexpr int LL = 512; EXPR; } break;   \
+    case 1024: { constexpr int LL = 1024; EXPR; } break; \
+    case 2048: { constexpr int LL = 2048; EXPR; } break; \
+    case 4096: { constexpr int LL = 4096; EXPR; } break; \
+    case 8192: { constexpr int LL = 8192; EXPR; } break; \
+    default: break;                               \
+    }
+
+} // namespace
+
+extern "C" {
+
+fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step, int template_width, int segment_len)
+{
+    if (!out) return FDAS_ERR_INVALID_ARG;
+    if (n_f < 1 || z_max < 0 || z_step < 1 || (z_max % z_step) != 0) return FDAS_ERR_INVALID_ARG;
+    if (template_width < 2 || (template_width & 1)) return FDAS_ERR_INVALID_ARG;
+    if (segment_len < 2 || (segment_len & (segment_len - 1))) return FDAS_ERR_INVALID_ARG;
+    if (!supported_L(segment_len)) return FDAS_ERR_UNSUPPORTED;
+    if (template_width > segment_len / 2) return FDAS_ERR_INVALID_ARG;
+    fdas_plan *p = (fdas_plan *)calloc(1, sizeof(fdas_plan));
+    if (!p) return FDAS_ERR_ALLOC;
+    p->n_f = n_f;
+    p->z_max = z_max;
+    p->z_step = z_step;
+    p->n_z = 2 * z_max / z_step + 1;
+    p->m = template_width;
+    p->L = segment_len;
+    p->S = segment_len - template_width;
+    p->n_seg = (n_f + p->S - 1) / p->S;
+    p->n_batch = 1;
+    cudaError_t e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
+    if (e == cudaSuccess) e = upload_twiddles(p->L, &p->d_tw);
+    if (e != cudaSuccess) {
+        fdas_status s = (e == cudaErrorMemoryAllocation) ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
+        (void)cudaGetLastError();
+        if (p->d_gperm) cudaFree(p->d_gperm);
+        if (p->d_tw) cudaFree(p->d_tw);
+        free(p);
+        return s;
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+fdas_status fdas_plan_set_batch(fdas_plan *p, int n_batch)
+{
+    if (!p || n_batch < 1) return FDAS_ERR_INVALID_ARG;
+    p->n_batch = n_batch;
+    return FDAS_OK;
+}
+
+fdas_status fdas_set_templates(fdas_plan *p, const float *h_templates)
+{
+    if (!p || !h_templates) return FDAS_ERR_INVALID_ARG;
+    const size_t bytes = sizeof(float2) * (size_t)p->n_z * (size_t)p->m;
+    float2 *d_h = nullptr;
+    cudaError_t e = cudaMalloc((void **)&d_h, bytes);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+    e = cudaMemcpy(d_h, h_templates, bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        const int L = p->L;
+        FDAS_DISPATCH_L(L, e = launch_template_fft<LL>(d_h, p->m, p->n_z, p->d_tw, p->d_gperm));
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    cudaFree(d_h);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->has_templates = true;
+    return FDAS_OK;
+}
+
+fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, void *cuda_stream)
+{
+    if (!p || !d_spectrum || !d_power) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_power & 3u)) return FDAS_ERR_INVALID_ARG;
+    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
+    ConvParams cp;
+    cp.spectrum = (const float2 *)d_spectrum;
+    cp.power = d_power;
+    cp.gperm = p->d_gperm;
+    cp.tw = p->d_tw;
+    cp.n_f = p->n_f;
+    cp.n_seg = p->n_seg;
+    cp.n_z = p->n_z;
+    cp.m = p->m;
+    cp.S = p->S;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaErrorInvalidValue;
+    const int L = p->L;
+    FDAS_DISPATCH_L(L, (e = launch_convolve<LL, 1>(cp, p->n_batch, st)));
+    p->last_launches = 1;
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return FDAS_OK;
+}
+
+fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_power, void *cuda_stream)
+{
+    if (!p || !h_spectrum || !h_power) return FDAS_ERR_INVALID_ARG;
+    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
+    const size_t sb = sizeof(float2) * (size_t)p->n_batch * (size_t)p->n_f;
+    const size_t pb = sizeof(float) * (size_t)p->n_batch * (size_t)p->n_z * (size_t)p->n_f;
+    cudaError_t e = cudaSuccess;
+    if (p->host_spec_bytes < sb) {
+        if (p->d_host_spec) cudaFree(p->d_host_spec);
+        p->d_host_spec = nullptr; p->host_spec_bytes = 0;
+        e = cudaMalloc(&p->d_host_spec, sb);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+        p->host_spec_bytes = sb;
+    }
+    if (p->host_power_bytes < pb) {
+        if (p->d_host_power) cudaFree(p->d_host_power);
+        p->d_host_power = nullptr; p->host_power_bytes = 0;
+        e = cudaMalloc((void **)&p->d_host_power, pb);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+        p->host_power_bytes = pb;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    fdas_status s = fdas_convolve(p, p->d_host_spec, p->d_host_power, cuda_stream);
+    if (s != FDAS_OK) return s;
+    e = cudaMemcpyAsync(h_power, p->d_host_power, pb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return FDAS_OK;
+}
+
+fdas_status fdas_plan_destroy(fdas_plan *p)
+{
+    if (!p) return FDAS_OK;
+    if (p->d_gperm) cudaFree(p->d_gperm);
+    if (p->d_tw) cudaFree(p->d_tw);
+    if (p->d_host_spec) cudaFree(p->d_host_spec);
+    if (p->d_host_power) cudaFree(p->d_host_power);
+    (void)cudaGetLastError();
+    free(p);
+    return FDAS_OK;
+}
+
+int fdas_plan_nz(const fdas_plan *p) { return p ? p->n_z : 0; }
+int fdas_plan_step(const fdas_plan *p) { return p ? p->S : 0; }
+int64_t fdas_plan_nseg(const fdas_plan *p) { return p ? p->n_seg : 0; }
+int fdas_plan_batch(const fdas_plan *p) { return p ? p->n_batch : 0; }
+int fdas_plan_last_launch_count(const fdas_plan *p) { return p ? p->last_launches : 0; }
+int fdas_plan_last_cuda_error(const fdas_plan *p) { return p ? p->last_cuda_error : -1; }
+
+const char *fdas_status_string(fdas_status s)
+{
+    switch (s) {
+    case FDAS_OK: return "FDAS_OK";
+    case FDAS_ERR_INVALID_ARG: return "FDAS_ERR_INVALID_ARG";
+    case FDAS_ERR_UNSUPPORTED: return "FDAS_ERR_UNSUPPORTED";
+    case FDAS_ERR_ALLOC: return "FDAS_ERR_ALLOC";
+    case FDAS_ERR_NO_TEMPLATES: return "FDAS_ERR_NO_TEMPLATES";
+    case FDAS_ERR_CUDA: return "FDAS_ERR_CUDA";
+    }
+    return "FDAS_ERR_UNKNOWN";
+}
+
+fdas_status fdas_debug_fft(int segment_len, int64_t n_seg, const void *d_in, void *d_out, int inverse)
+{
+    if (!d_in || !d_out || n_seg < 0) return FDAS_ERR_INVALID_ARG;
+    if (!supported_L(segment_len)) return FDAS_ERR_UNSUPPORTED;
+    if (n_seg == 0) return FDAS_OK;
+    float2 *d_tw = nullptr;
+    cudaError_t e = upload_twiddles(segment_len, &d_tw);
+    if (e == cudaSuccess) {
+        FDAS_DISPATCH_L(segment_len, e = launch_debug_fft<LL>(n_seg, (const float2 *)d_in, (float2 *)d_out, d_tw, inverse));
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (d_tw) cudaFree(d_tw);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    return FDAS_OK;
+}
+
+const char *fdas_version(void) { return "libfdas sm_100a " __DATE__; }
+
+} // extern "C"
