@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- FDAS matched-filter hot path on B200: (z,r) points/s and fraction of the roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+A "step" is one fdas_convolve over one batch of synthetic spectra: segment load, forward FFT,
+then for every z multiply / inverse FFT / trim / power / write (DESIGN.md rows a1-a6).  The default
+workload is BASELINE.json configs[2] (the config its metric is quoted on): N_f = 2^22 bins, 201
+z-trials, m = 512, L = 4096.  Prints ONE JSON line (rank 0).  For N > 1 (torchrun) every rank runs
+the same workload on its own seeded spectra -- the path shards by spectrum with no exchange step --
+and `value` is all ranks' points over the slowest rank's device time ("scaling": "weak").
+
+`--impl reference`: there is no reference implementation for this paper; this arm times the
+double-precision oracle (oracle/, the plain statement of eq.(2)) on the host cores, on a bounded
+sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fdas_conv_zr_points_per_s"
+UNIT = "points/s"
+FP32_LANES_PER_SM = 128  # B200: 4 SMSPs x 32 FP32 lanes, 2 flops per FMA
+N_SM = 148
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the hot kernel, from the committed
+# `ncu --set full` capture named here (None until a capture exists for that workload).
+NCU_TRAFFIC = {
+    # "C3": (bytes, "profiles/r1_c3_full.md"),
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5 (4 = sweep pair --pair)")
+    ap.add_argument("--pair", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the plane the oracle is timed on (0 = auto)")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+def algorithmic_work(wl, S, n_seg):
+    """Per launch: HBM bytes and nominal FFT flops."""
+    L = wl.seg_len
+    out_b = 4 * wl.n_batch * wl.n_z * wl.n_f
+    in_b = 8 * wl.n_batch * n_seg * L          # every segment loads L bins (overlap re-read included)
+    tpl_b = 8 * wl.n_z * L                     # template bank once (L2 resident afterwards)
+    fft = 5.0 * L * np.log2(L)
+    flops = wl.n_batch * n_seg * (1 + wl.n_z) * fft
+    return out_b + in_b + tpl_b, flops
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(self.index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [l.split(", ") for (ts, l) in self.lines if t0 - 0.05 <= ts <= t1 + 0.15]
+        if not rows:
+            rows = [l.split(", ") for (_, l) in self.lines]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.strip().lower() == "active":
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w": float(np.median(pw)) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(args, rank):
+    from paper_1711_10855_b200 import workload
+    c = args.config
+    wl = workload.make_config(c, pair=args.pair if c == 4 else 0)
+    if rank:  # other ranks: same shape, own noise (weak scaling over independent spectra)
+        wl.spectrum = workload.noise_spectrum(wl.n_f, workload.SEED_BASE + 1000 * c + 7919 * rank, wl.n_batch)
+    return wl
+
+
+def cpu_baseline(wl, rows=0, target_s=15.0):
+    """The oracle's direct sum (eq.(2)) timed on the host cores on `rows` full rows of the plane."""
+    import oracle
+    H = wl.templates.astype(np.complex128)
+    A = wl.spectrum[0]
+    nthr = oracle.num_threads()
+    mid = wl.n_z // 2
+    t0 = time.perf_counter()
+    oracle.direct(A, H, rows=(mid, mid + 1))
+    t1 = time.perf_counter() - t0
+    if rows <= 0:
+        rows = int(max(1, min(wl.n_z, round(target_s / max(t1, 1e-4)))))
+    r0 = max(0, min(wl.n_z - rows, mid - rows // 2))
+    t0 = time.perf_counter()
+    oracle.direct(A, H, rows=(r0, r0 + rows))
+    dt = time.perf_counter() - t0
+    pts = rows * wl.n_f
+    return {"value": pts / dt, "unit": UNIT, "cores": nthr, "kind": "oracle",
+            "sample": f"rows {r0}..{r0 + rows - 1} of {wl.n_z} x all {wl.n_f} columns of spectrum 0 "
+                      f"(double direct sum of eq.(2), {rows * wl.n_f * wl.m:.3g} complex MACs in {dt:.2f} s)",
+            "seconds": dt}, pts, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = make_workload(args, 0)
+    S = wl.seg_len - wl.m
+    # bounded sample per step: calibrate rows so the whole run ends within a few minutes
+    base, _, _ = cpu_baseline(wl, rows=1)
+    per_row = base["seconds"]
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    rows = int(max(1, min(wl.n_z, budget / max(per_row, 1e-4))))
+    for _ in range(args.warmup):
+        cpu_baseline(wl, rows=rows)
+    tot_pts, tot_t, last = 0, 0.0, None
+    for _ in range(args.steps):
+        last, pts, dt = cpu_baseline(wl, rows=rows)
+        tot_pts += pts
+        tot_t += dt
+    value = tot_pts / tot_t
+    last["value"] = value
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"{wl.name}: N_f={wl.n_f} n_z={wl.n_z} m={wl.m} L={wl.seg_len}",
+                      "note": "no reference implementation exists; this is the CPU oracle on a bounded sample"},
+           "cpu_baseline": last, "gpu_launches": 0,
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1711_10855_b200 import binding
+
+    binding.lib()  # fail loudly if the CUDA extension is missing
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = make_workload(args, rank)
+    plan = binding.Plan(wl.n_f, wl.z_max, wl.z_step, wl.m, wl.seg_len, n_batch=wl.n_batch)
+    plan.set_templates(wl.templates)
+    S, n_seg = plan.step, plan.n_seg
+    bytes_alg, flops_alg = algorithmic_work(wl, S, n_seg)
+    points = wl.points
+
+    # inputs resident in HBM; rotate over enough distinct spectra to exceed the 126 MB L2
+    from paper_1711_10855_b200 import workload
+    spec_bytes = wl.spectrum.nbytes
+    n_rot = max(1, min(8, int(np.ceil(200e6 / spec_bytes))))
+    d_specs = [torch.from_numpy(wl.spectrum).cuda()]
+    for i in range(1, n_rot):
+        d_specs.append(torch.from_numpy(
+            workload.noise_spectrum(wl.n_f, workload.SEED_BASE + 31 * i + 7919 * rank, wl.n_batch)).cuda())
+    d_pow = torch.empty((wl.n_batch, wl.n_z, wl.n_f), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.Stream()
+
+    with torch.cuda.stream(stream):
+        for i in range(max(3, args.warmup)):
+            plan.convolve(d_specs[i % n_rot], d_pow, stream=stream)
+    barrier()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    t_wall0 = time.time()
+    launches = 0
+    ev[0].record(stream)
+    for i in range(args.steps):
+        plan.convolve(d_specs[i % n_rot], d_pow, stream=stream)
+        launches += plan.last_launch_count
+        ev[i + 1].record(stream)
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    ms_per_step = total_ms_max / args.steps
+    value = world * points * args.steps / (total_ms_max * 1e-3)
+
+    # e2e: host buffers through the C ABI, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        h_spec = torch.from_numpy(wl.spectrum).pin_memory()
+        h_pow = torch.empty((wl.n_batch, wl.n_z, wl.n_f), dtype=torch.float32).pin_memory()
+        e2e_steps = max(1, min(args.steps, 5))
+        plan.convolve_host(h_spec, h_pow, stream=stream)  # warm-up: allocates the plan's staging buffers
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(e2e_steps):
+            plan.convolve_host(h_spec, h_pow, stream=stream)
+        e1.record(stream)
+        barrier()
+        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * points * e2e_steps / (float(te.item()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(h_spec.numel() * 8), "d2h_bytes_per_step": int(h_pow.numel() * 4),
+               "steps": e2e_steps, "ms_per_step": float(te.item()) / e2e_steps}
+        del h_pow
+
+    if rank == 0:
+        pk = peaks()
+        kern_ms = float(np.mean(per_launch_ms))
+        fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s at max clock
+        ach_tf = flops_alg / (kern_ms * 1e-3) / 1e12
+        ach_gb = bytes_alg / (kern_ms * 1e-3) / 1e9
+        t_alu = flops_alg / (fp32_peak * 1e12)
+        t_hbm = bytes_alg / (pk["hbm_gbs"] * 1e9)
+        alu_binds = t_alu >= t_hbm
+        traffic = NCU_TRAFFIC.get(wl.name.split("[")[0], (None, None))
+        roofline = {
+            "bound": "alu" if alu_binds else "hbm",
+            "achieved": ach_tf if alu_binds else ach_gb,
+            "peak": fp32_peak if alu_binds else pk["hbm_gbs"],
+            "unit": "TFLOP/s" if alu_binds else "GB/s",
+            "frac": (ach_tf / fp32_peak) if alu_binds else (ach_gb / pk["hbm_gbs"]),
+            "traffic": traffic[0], "traffic_source": traffic[1],
+            "kernel": f"fdas_convolve_kernel<{wl.seg_len}>", "kernel_ms": kern_ms, "kernel_ms_min": float(np.min(per_launch_ms)),
+            "flops_per_launch": flops_alg, "bytes_per_launch": bytes_alg,
+            "alu": {"achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach_tf / fp32_peak,
+                    "peak_def": f"{N_SM} SMs x {FP32_LANES_PER_SM} lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (nominal; flops = 5 L log2 L per transform)"},
+            "hbm": {"achieved": ach_gb, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": ach_gb / pk["hbm_gbs"],
+                    "peak_def": f"MEASURED_PEAKS.json hbm_gbs ({pk['source']})"},
+        }
+        if clocks and clocks.get("sm_mhz"):
+            at_clock = N_SM * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12
+            roofline["alu"]["frac_at_measured_clock"] = ach_tf / at_clock
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+               "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f32", "data": "synthetic",
+               "config": {"workload": f"{wl.name}: N_f={wl.n_f} n_z={wl.n_z} m={wl.m} L={wl.seg_len} batch={wl.n_batch} per GPU",
+                          "segments": int(n_seg), "step_S": int(S),
+                          "l2": f"output plane {d_pow.numel() * 4 / 1e9:.2f} GB >> 126 MB L2; inputs rotate over {n_rot} spectra "
+                                f"({n_rot * spec_bytes / 1e6:.0f} MB) so no flush is needed",
+                          "parallelism": f"{world} x independent spectra (no collective)"},
+               "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+        if not args.no_cpu_baseline and world >= 1:
+            cb, _, _ = cpu_baseline(wl, rows=args.cpu_rows)
+            cb.pop("seconds", None)
+            out["cpu_baseline"] = cb
+        print(json.dumps(out))
+    plan.destroy()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

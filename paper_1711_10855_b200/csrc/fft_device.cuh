@@ -21,6 +21,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "butterflies_gen.cuh"
+
 namespace fdas {
 
 template <int L_, int E_, int R0_, int R1_, int R2_, int R3_>
@@ -52,99 +54,33 @@ template <> struct Cfg<8192> : CfgT<8192, 16, 16, 8, 8, 8> {};
 // ---------------------------------------------------------------------------------------------
 // complex helpers
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Packed FP32x2 arithmetic on (re, im) pairs: one FMUL2 + one FFMA2 per complex product; the swap
+// and the per-half sign are operand modifiers in SASS (.F32x2.LO_HI, .NP / .PN, .F32 broadcast).
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 {
-    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+    const float2 p = __fmul2_rn(a, make_float2(b.x, b.x));
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-b.y, b.y), p);
 }
 // a * conj(b)
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b)
 {
-    return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
-}
-// multiply by -i (forward quarter turn) or +i (inverse)
-template <bool INV> __device__ __forceinline__ float2 rot90(float2 a)
-{
-    return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
-}
-
-// cos(2 pi k / 32), k = 0..8 (double-rounded literals); other angles by symmetry at compile time.
-__host__ __device__ constexpr float cos32(int k)
-{
-    // k in [0, 32)
-    k &= 31;
-    if (k > 16) k = 32 - k;          // cos is even about pi
-    bool neg = false;
-    if (k > 8) { k = 16 - k; neg = true; }
-    float c = k == 0 ? 1.0f
-            : k == 1 ? 0.98078528040323044913f
-            : k == 2 ? 0.92387953251128675613f
-            : k == 3 ? 0.83146961230254523708f
-            : k == 4 ? 0.70710678118654752440f
-            : k == 5 ? 0.55557023301960222474f
-            : k == 6 ? 0.38268343236508977173f
-            : k == 7 ? 0.19509032201612826785f
-            : 0.0f;
-    return neg ? -c : c;
-}
-__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
-
-// v * w_R^j (forward) or v * conj(w_R^j) (inverse), R <= 32, j compile-time.
-template <int R, int J, bool INV> __device__ __forceinline__ float2 mul_wconst(float2 v)
-{
-    constexpr int k = ((J * (32 / R)) % 32 + 32) % 32; // angle in 32nds of a turn
-    if constexpr (k == 0) return v;
-    else if constexpr (k == 8) return rot90<INV>(v);
-    else if constexpr (k == 16) return make_float2(-v.x, -v.y);
-    else if constexpr (k == 24) return rot90<!INV>(v);
-    else {
-        constexpr float c = cos32(k);
-        constexpr float s = INV ? sin32(k) : -sin32(k); // w = c + i s with s = -sin for the forward sign
-        return make_float2(v.x * c - v.y * s, v.x * s + v.y * c);
-    }
+    const float2 p = __fmul2_rn(a, make_float2(b.x, b.x));
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(b.y, -b.y), p);
 }
 
 // In-register DFT of R points, natural order in and out.  INV = conjugate twiddles (unnormalised).
+// The bodies are generated (gen_butterflies.py) in packed FP32x2 form.
 template <int R, bool INV> struct Dft;
 template <bool INV> struct Dft<1, INV> { __device__ __forceinline__ static void run(float2 *) {} };
-template <bool INV> struct Dft<2, INV> {
-    __device__ __forceinline__ static void run(float2 *v)
-    {
-        float2 a = cadd(v[0], v[1]), b = csub(v[0], v[1]);
-        v[0] = a; v[1] = b;
-    }
-};
-template <bool INV> struct Dft<4, INV> {
-    __device__ __forceinline__ static void run(float2 *v)
-    {
-        float2 a0 = cadd(v[0], v[2]), a1 = csub(v[0], v[2]);
-        float2 a2 = cadd(v[1], v[3]), a3 = rot90<INV>(csub(v[1], v[3]));
-        v[0] = cadd(a0, a2); v[2] = csub(a0, a2);
-        v[1] = cadd(a1, a3); v[3] = csub(a1, a3);
-    }
-};
-// radix-2 split (decimation in frequency): a_j = x_j + x_{j+R/2}, b_j = (x_j - x_{j+R/2}) w_R^j,
-// X_{2k} = DFT_{R/2}(a)_k, X_{2k+1} = DFT_{R/2}(b)_k.
-template <int R, bool INV> struct Dft {
-    template <int J> __device__ __forceinline__ static void split(float2 *v, float2 *a, float2 *b)
-    {
-        if constexpr (J < R / 2) {
-            a[J] = cadd(v[J], v[J + R / 2]);
-            b[J] = mul_wconst<R, J, INV>(csub(v[J], v[J + R / 2]));
-            split<J + 1>(v, a, b);
-        }
-    }
-    __device__ __forceinline__ static void run(float2 *v)
-    {
-        float2 a[R / 2], b[R / 2];
-        split<0>(v, a, b);
-        Dft<R / 2, INV>::run(a);
-        Dft<R / 2, INV>::run(b);
-#pragma unroll
-        for (int k = 0; k < R / 2; ++k) { v[2 * k] = a[k]; v[2 * k + 1] = b[k]; }
-    }
-};
+#define FDAS_DFT_SPEC(R)                                                                                   \
+    template <bool INV> struct Dft<R, INV> {                                                               \
+        __device__ __forceinline__ static void run(float2 *v) { if (INV) dft##R##_inv(v); else dft##R##_fwd(v); } \
+    };
+FDAS_DFT_SPEC(2)
+FDAS_DFT_SPEC(4)
+FDAS_DFT_SPEC(8)
+FDAS_DFT_SPEC(16)
+#undef FDAS_DFT_SPEC
 
 // ---------------------------------------------------------------------------------------------
 // layouts
