@@ -16,20 +16,9 @@
 
 #include "../../include/fdas.h"
 #include "fft_device.cuh"
+#include "convolve_tmem.cuh"
 
 namespace fdas {
-
-struct ConvParams {
-    const float2 *__restrict__ spectrum; // [n_batch][n_f]
-    float *__restrict__ power;           // [n_batch][n_z][n_f]
-    const float4 *__restrict__ gperm;    // [n_z][E/2][NT] : template spectra in register order
-    const float2 *__restrict__ tw;       // [L] : w_L^j
-    int64_t n_f;
-    int64_t n_seg;
-    int n_z;
-    int m;
-    int S;
-};
 
 // Inverse-pass twiddles kept in registers across the z loop (they do not depend on z): the
 // paper's "reuse already calculated twiddle factors" taken to its limit.
@@ -238,6 +227,7 @@ struct fdas_plan {
     float4 *d_gperm;   // n_z * L complex64
     float2 *d_tw;      // L complex64
     bool has_templates;
+    int variant;       // 2: TMEM-resident kernel (default); 1: register-resident kernel (FDAS_VARIANT=1)
     int last_cuda_error;
     int last_launches;
     // buffers of fdas_convolve_host
@@ -288,6 +278,23 @@ template <int L, int MINB> cudaError_t launch_convolve(const ConvParams &cp, int
     const int64_t blocks = cp.n_seg * n_batch;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     kern<<<(unsigned)blocks, Cfg<L>::NT, smem_bytes<L>(), st>>>(cp);
+    return cudaGetLastError();
+}
+
+template <int L> size_t smem_bytes_tmem() { return smem_bytes<L>() + sizeof(float2) * (size_t)L; }
+
+template <int L> cudaError_t launch_convolve_tmem(const ConvParams &cp, int n_batch, cudaStream_t st)
+{
+    auto kern = fdas_convolve_tmem_kernel<L>;
+    static bool attr_done = false; // per instantiation; benign race (idempotent)
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes_tmem<L>());
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int64_t blocks = cp.n_seg * n_batch;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    kern<<<(unsigned)blocks, Cfg<L>::NT, smem_bytes_tmem<L>(), st>>>(cp);
     return cudaGetLastError();
 }
 
@@ -342,6 +349,10 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
     p->S = segment_len - template_width;
     p->n_seg = (n_f + p->S - 1) / p->S;
     p->n_batch = 1;
+    {
+        const char *v = getenv("FDAS_VARIANT");
+        p->variant = (v && v[0] == '1') ? 1 : 2;
+    }
     cudaError_t e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
     if (e == cudaSuccess) e = upload_twiddles(p->L, &p->d_tw);
     if (e != cudaSuccess) {
@@ -400,7 +411,11 @@ fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
-    FDAS_DISPATCH_L(L, (e = launch_convolve<LL, 1>(cp, p->n_batch, st)));
+    if (p->variant == 1) {
+        FDAS_DISPATCH_L(L, (e = launch_convolve<LL, 1>(cp, p->n_batch, st)));
+    } else {
+        FDAS_DISPATCH_L(L, (e = launch_convolve_tmem<LL>(cp, p->n_batch, st)));
+    }
     p->last_launches = 1;
     if (e != cudaSuccess) return cuda_fail(p, e);
     return FDAS_OK;
