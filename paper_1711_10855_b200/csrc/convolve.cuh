@@ -1,0 +1,304 @@
+// convolve.cuh -- the FDAS hot kernel (steps a1..a6 of DESIGN.md) for sm_100a.
+//
+// One CTA owns one (batch item, segment) and loops over all n_z templates ("for every matched
+// filter": multiply, inverse FFT, store).  Where the loop-invariant data live:
+//   * the forward-transformed segment X and the per-thread inverse twiddles of the passes after the
+//     first live in TENSOR MEMORY (tcgen05.st once per segment, tcgen05.ld per z): TMEM is a 256 KB
+//     per-SM array with its own data path (measured 930 B/clk/SM), so these reads cost neither
+//     registers nor LSU / shared-memory bandwidth;
+//   * G_z is brought from L2 into shared memory by the bulk-copy engine (cp.async.bulk, one elected
+//     thread, mbarrier completion) one z ahead and read with conflict-free LDS.128;
+//   * the working set v, the pass-0 twiddles and addressing stay in registers (<= 128 registers, two
+//     256-thread CTAs per SM at L = 4096).
+// The inverse transform (fft_device.cuh, "Inverse transform of the hot loop") exchanges data once
+// by warp shuffles and once (L = 8192: twice) through shared memory; one barrier per exchange.
+#pragma once
+#include "fft_device.cuh"
+#include "sm100_ptx.cuh"
+
+namespace fdas {
+
+// ---------------------------------------------------------------------------------------------
+// inverse passes P-1 ... 0 on v (layout P-1, template already multiplied in).  TW supplies the
+// multipliers of pass P-2 (E entries, entry j*Rb is unused) and, for P == 4, of pass 1; tw0 holds
+// w_L^{d t} for pass 0.  All multipliers are applied conjugated (cmulc).  `hook` runs right after
+// the first block barrier.  P == 3: bufa alternates between calls (one barrier per call).
+// ---------------------------------------------------------------------------------------------
+template <class C, class TW, class Hook>
+__device__ __forceinline__ void inverse_transform(float2 *v, float2 *bufa, float2 *bufb, const InvAddr<C> &A, const float2 *tw0,
+                                                  TW &tws, int lane, Hook &&hook)
+{
+    using I = InvCfg<C>;
+    constexpr int E = C::E;
+#pragma unroll
+    for (int i = 0; i < I::NB; ++i) Dft<I::Ra, true>::run(v + i * I::Ra);
+    float2 twa[E];
+    tws.issue_a(twa);
+    float2 w[E];
+    inv_shuffle<C>(v, w, lane);
+    tws.wait_a(twa);
+#pragma unroll
+    for (int j = 0; j < I::NA; ++j)
+#pragma unroll
+        for (int tau = 1; tau < I::Rb; ++tau) w[j * I::Rb + tau] = cmulc(w[j * I::Rb + tau], twa[j * I::Rb + tau]);
+#pragma unroll
+    for (int j = 0; j < I::NA; ++j) Dft<I::Rb, true>::run(w + j * I::Rb);
+    inv_write_a<C>(bufa, A.wa, w);
+    if constexpr (C::P == 3) {
+        __syncthreads();
+        hook();
+#pragma unroll
+        for (int k = 0; k < C::R(0); ++k) v[k] = bufa[A.ra + k * I::STR0];
+    } else {
+        constexpr int R1 = C::R(1), B1 = E / R1;
+        float2 twm[8];
+        tws.issue_m(twm);
+        __syncthreads();
+        hook();
+#pragma unroll
+        for (int b = 0; b < B1; ++b)
+#pragma unroll
+            for (int k = 0; k < R1; ++k) v[b * R1 + k] = bufa[A.ra + (b * I::KK * R1 + k) * I::STRX];
+        tws.wait_m(twm);
+#pragma unroll
+        for (int d = 1; d < R1; ++d)
+#pragma unroll
+            for (int b = 0; b < B1; ++b) v[b * R1 + d] = cmulc(v[b * R1 + d], twm[d]);
+#pragma unroll
+        for (int b = 0; b < B1; ++b) Dft<R1, true>::run(v + b * R1);
+#pragma unroll
+        for (int b = 0; b < B1; ++b)
+#pragma unroll
+            for (int n = 0; n < R1; ++n) bufb[A.wb + I::KK * b * I::STR0 + n * I::Q] = v[b * R1 + n];
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < C::R(0); ++k) v[k] = bufb[A.rb + k * I::STR0];
+    }
+#pragma unroll
+    for (int d = 1; d < C::R(0); ++d) v[d] = cmulc(v[d], tw0[d]);
+    Dft<C::R(0), true>::run(v);
+}
+
+// multipliers read from the w_L table in global memory (set-up code, debug kernel)
+template <class C> struct TwLdg {
+    const float2 *__restrict__ tw;
+    int t;
+    __device__ __forceinline__ void issue_a(float2 *o) const
+    {
+        using I = InvCfg<C>;
+#pragma unroll
+        for (int j = 0; j < I::NA; ++j) {
+            o[j * I::Rb] = make_float2(1.f, 0.f);
+#pragma unroll
+            for (int tau = 1; tau < I::Rb; ++tau) o[j * I::Rb + tau] = __ldg(tw + inv_twa_index<C>(t, j, tau));
+        }
+    }
+    __device__ __forceinline__ void wait_a(float2 *) const {}
+    __device__ __forceinline__ void issue_m(float2 *o) const
+    {
+        if constexpr (C::P == 4) {
+            const int u = tw_unit<C, 1>(t);
+            o[0] = make_float2(1.f, 0.f);
+#pragma unroll
+            for (int d = 1; d < C::R(1); ++d) o[d] = __ldg(tw + d * u);
+        }
+    }
+    __device__ __forceinline__ void wait_m(float2 *) const {}
+};
+
+// tensor-memory geometry: per thread (TMEM lane) a block of columns X | TWA [| TWM]
+template <class C> struct TmemCfg {
+    static constexpr int SLOTS = (C::NT + 127) / 128;          // warps sharing a 32-lane quarter
+    static constexpr int X_OFF = 0, TWA_OFF = 32, TWM_OFF = 64;
+    static constexpr int SLOT_COLS = C::P == 3 ? 64 : 128;
+    static constexpr int NCOLS_RAW = SLOT_COLS * SLOTS;
+    static constexpr int NCOLS = NCOLS_RAW <= 32 ? 32 : NCOLS_RAW <= 64 ? 64 : NCOLS_RAW <= 128 ? 128 : NCOLS_RAW <= 256 ? 256 : 512;
+    static constexpr int MINB = (512 / C::NT) > 0 ? (512 / C::NT) : 1; // CTAs per SM at 128 registers
+    static_assert(2 * C::E <= 32, "a segment slice or a twiddle block is at most 32 columns");
+    static_assert(NCOLS_RAW <= 512 && NCOLS * MINB <= 512, "tensor memory holds 512 columns per SM");
+};
+
+// multipliers parked in tensor memory
+template <class C> struct TwTmem {
+    uint32_t addr; // TMEM address of this thread's column block
+    __device__ __forceinline__ void issue_a(float2 *o) const
+    {
+        ptx::tmem_ld16(addr + TmemCfg<C>::TWA_OFF, o);
+        if constexpr (C::E > 8) ptx::tmem_ld16(addr + TmemCfg<C>::TWA_OFF + 16, o + 8);
+    }
+    __device__ __forceinline__ void wait_a(float2 *o) const
+    {
+        ptx::tmem_wait_ld8(o);
+        if constexpr (C::E > 8) ptx::tmem_wait_ld8(o + 8);
+    }
+    __device__ __forceinline__ void issue_m(float2 *o) const
+    {
+        if constexpr (C::P == 4) ptx::tmem_ld16(addr + TmemCfg<C>::TWM_OFF, o);
+    }
+    __device__ __forceinline__ void wait_m(float2 *o) const
+    {
+        if constexpr (C::P == 4) ptx::tmem_wait_ld8(o);
+    }
+};
+
+// forward transform of v (natural order, v[d] = x[d*NT + t]) into layout P-1 of the inverse:
+// the decimation-in-frequency passes of fft_device.cuh followed by one re-layout through buf0.
+template <class C> __device__ __forceinline__ void forward_to_inv_layout(float2 *v, float2 *buf0, float2 *buf1,
+                                                                         const float2 *__restrict__ tw, int t)
+{
+    using I = InvCfg<C>;
+    constexpr int RL = C::R(C::P - 1), BL = C::E / RL;
+    fwd_from<C, 0>(v, buf0, buf1, tw, t);
+    __syncthreads();
+#pragma unroll
+    for (int b = 0; b < BL; ++b)
+#pragma unroll
+        for (int d = 0; d < RL; ++d) buf0[nat_freq<C>(t, b, d)] = v[b * RL + d];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < I::NB; ++i)
+#pragma unroll
+        for (int k = 0; k < I::Ra; ++k) v[i * I::Ra + k] = buf0[inv_freq<C>(t, i, k)];
+}
+
+struct ConvParams {
+    const float2 *__restrict__ spectrum; // [n_batch][n_f]
+    float *__restrict__ power;           // [n_batch][n_z][n_f]
+    const float4 *__restrict__ gperm;    // [n_z][E/2][NT] : template spectra in register order
+    const float2 *__restrict__ tw;       // [L] : w_L^j
+    int64_t n_f;
+    int64_t n_seg;
+    int n_z;
+    int m;
+    int S;
+};
+
+template <class C> constexpr size_t conv_smem_bytes()
+{
+    return 2 * sizeof(float2) * (size_t)InvCfg<C>::BUF_ELEMS + sizeof(float2) * (size_t)C::L;
+}
+
+template <int L>
+__global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convolve_kernel(const ConvParams p)
+{
+    using C = Cfg<L>;
+    using I = InvCfg<C>;
+    using TC = TmemCfg<C>;
+    constexpr int E = C::E, NT = C::NT;
+    constexpr uint32_t G_BYTES = (uint32_t)L * 8u;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *buf0 = reinterpret_cast<float2 *>(smem_raw);
+    float2 *buf1 = buf0 + I::BUF_ELEMS;
+    float4 *gs = reinterpret_cast<float4 *>(buf1 + I::BUF_ELEMS); // [E/2][NT]
+    __shared__ __align__(8) uint64_t g_bar;
+    __shared__ uint32_t tmem_slot;
+
+    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+    const int64_t seg = blockIdx.x % p.n_seg;
+    const int64_t bi = blockIdx.x / p.n_seg;
+
+    if (t == 0) {
+        ptx::mbar_init(&g_bar, 1);
+        ptx::mbar_fence_init();
+    }
+    if (warp == 0) ptx::tmem_alloc<TC::NCOLS>(&tmem_slot);
+    ptx::tmem_fence_before_sync();
+    __syncthreads();
+    ptx::tmem_fence_after_sync();
+    if (t == 0) { // template spectrum of z = 0 (a3), in flight during the forward transform
+        ptx::mbar_expect_tx(&g_bar, G_BYTES);
+        ptx::bulk_g2s(gs, p.gperm, G_BYTES, &g_bar);
+    }
+    const uint32_t tm_addr = tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(TC::SLOT_COLS * (warp >> 2));
+
+    // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
+    float2 v[E];
+    {
+        const float2 *__restrict__ A = p.spectrum + bi * p.n_f;
+        const int64_t base = seg * p.S - p.m / 2;
+#pragma unroll
+        for (int d = 0; d < E; ++d) {
+            const int64_t k = base + d * NT + t;
+            v[d] = (k >= 0 && k < p.n_f) ? __ldg(A + k) : make_float2(0.f, 0.f);
+        }
+    }
+    // a2: forward FFT, once per segment (eq.(3)); the result is parked in tensor memory
+    forward_to_inv_layout<C>(v, buf0, buf1, p.tw, t);
+    ptx::tmem_st16(tm_addr + TC::X_OFF, v);
+    if constexpr (E > 8) ptx::tmem_st16(tm_addr + TC::X_OFF + 16, v + 8);
+
+    // inverse multipliers (independent of z): pass 0 in registers, the others in tensor memory
+    float2 tw0[C::R(0)];
+    {
+        tw0[0] = make_float2(1.f, 0.f);
+#pragma unroll
+        for (int d = 1; d < C::R(0); ++d) tw0[d] = __ldg(p.tw + d * t);
+        TwLdg<C> src{p.tw, t};
+        float2 w[16];
+#pragma unroll
+        for (int d = 0; d < 16; ++d) w[d] = make_float2(1.f, 0.f);
+        src.issue_a(w);
+        ptx::tmem_st16(tm_addr + TC::TWA_OFF, w);
+        if constexpr (E > 8) ptx::tmem_st16(tm_addr + TC::TWA_OFF + 16, w + 8);
+        if constexpr (C::P == 4) {
+            src.issue_m(w);
+            ptx::tmem_st16(tm_addr + TC::TWM_OFF, w);
+        }
+    }
+    ptx::tmem_wait_st();
+    __syncthreads(); // the forward transform's last reads of buf0 are done before the z loop writes it
+
+    const InvAddr<C> A = inv_addr<C>(t);
+    TwTmem<C> tws{tm_addr};
+
+    const int64_t col0 = seg * p.S - p.m + t;                 // column of y[t]
+    float *__restrict__ prow = p.power + bi * p.n_z * p.n_f;  // row 0 of this batch item
+    const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
+    const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
+    const int d0 = p.m / NT;
+
+    for (int z = 0; z < p.n_z; ++z) {
+        // a3: pointwise multiply by the transformed template ("convolution in the Fourier domain")
+        float2 X[E];
+        ptx::tmem_ld16(tm_addr + TC::X_OFF, X);
+        if constexpr (E > 8) ptx::tmem_ld16(tm_addr + TC::X_OFF + 16, X + 8);
+        ptx::mbar_wait(&g_bar, (uint32_t)(z & 1));
+        ptx::tmem_wait_ld8(X);
+        if constexpr (E > 8) ptx::tmem_wait_ld8(X + 8);
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) {
+            const float4 g = gs[q * NT + t];
+            v[2 * q] = cmul(X[2 * q], make_float2(g.x, g.y));
+            v[2 * q + 1] = cmul(X[2 * q + 1], make_float2(g.z, g.w));
+        }
+        // a4: inverse FFT.  After its first block barrier every thread has consumed G_z, so the
+        // elected thread starts the bulk copy of G_{z+1} into the same stage.
+        float2 *bufa = (C::P == 3 && (z & 1)) ? buf1 : buf0;
+        inverse_transform<C>(v, bufa, buf1, A, tw0, tws, lane, [&]() {
+            if (t == 0 && z + 1 < p.n_z) {
+                ptx::mbar_expect_tx(&g_bar, G_BYTES);
+                ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)(z + 1) * G_BYTES, G_BYTES, &g_bar);
+            }
+        });
+        // a5 + a6: trim, power, coalesced store
+        float *__restrict__ out = prow + (int64_t)z * p.n_f + col0;
+        if (fast) {
+#pragma unroll
+            for (int d = 0; d < E; ++d) {
+                if (d >= 4 || d >= d0) __stcs(out + d * NT, v[d].x * v[d].x + v[d].y * v[d].y);
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < E; ++d) {
+                const int pidx = d * NT + t;
+                const int64_t col = col0 + d * NT;
+                if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = v[d].x * v[d].x + v[d].y * v[d].y;
+            }
+        }
+    }
+    ptx::tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) ptx::tmem_free<TC::NCOLS>(tmem_slot);
+}
+
+} // namespace fdas

@@ -16,135 +16,14 @@
 
 #include "../../include/fdas.h"
 #include "fft_device.cuh"
-#include "convolve_tmem.cuh"
+#include "convolve.cuh"
 
 namespace fdas {
 
-// Inverse-pass twiddles kept in registers across the z loop (they do not depend on z): the
-// paper's "reuse already calculated twiddle factors" taken to its limit.
-template <class C> struct InvTw { float2 w[C::P - 1][C::E]; };
-
-template <class C, int I> __device__ __forceinline__ void load_inv_tw(InvTw<C> &T, const float2 *__restrict__ tw, int t)
-{
-    if constexpr (I < C::P - 1) {
-        const int u = tw_unit<C, I>(t);
-#pragma unroll
-        for (int d = 1; d < C::R(I); ++d) T.w[I][d] = __ldg(tw + d * u);
-        load_inv_tw<C, I + 1>(T, tw, t);
-    }
-}
-
-// Inverse passes: v enters in layout I+1 with its butterflies done; exchange to layout I, apply the
-// conjugate twiddles, butterfly; recurse down to pass 0.  One barrier per exchange; the two
-// buffers alternate so a buffer is rewritten only after a later barrier.
-template <class C, int I> __device__ __forceinline__ void inv_down(float2 *v, float2 *buf0, float2 *buf1,
-                                                                    const InvTw<C> &T, const int *bases)
-{
-    constexpr int R = C::R(I), B = C::E / R;
-    float2 *buf = (I & 1) ? buf1 : buf0;
-    sm_write<C, I + 1>(buf, bases[I + 1], v);
-    __syncthreads();
-    sm_read<C, I>(buf, bases[I], v);
-#pragma unroll
-    for (int d = 1; d < R; ++d)
-#pragma unroll
-        for (int b = 0; b < B; ++b) v[b * R + d] = cmulc(v[b * R + d], T.w[I][d]);
-    butterflies<C, I, true>(v);
-    if constexpr (I > 0) inv_down<C, I - 1>(v, buf0, buf1, T, bases);
-}
-
-template <class C, int I> __device__ __forceinline__ void fill_bases(int *bases, int t)
-{
-    bases[I] = lay_base<C, I>(t);
-    if constexpr (I + 1 < C::P) fill_bases<C, I + 1>(bases, t);
-}
-
 // -------------------------------------------------------------------------------------------
-// Hot kernel: steps a1..a6 of DESIGN.md for one (batch item, segment), all z.
-// -------------------------------------------------------------------------------------------
-template <int L, int MINB>
-__global__ void __launch_bounds__(Cfg<L>::NT, MINB) fdas_convolve_kernel(const ConvParams p)
-{
-    using C = Cfg<L>;
-    constexpr int E = C::E, NT = C::NT;
-    extern __shared__ float2 smem[];
-    float2 *buf0 = smem, *buf1 = smem + C::SMEM_ELEMS;
-    const int t = threadIdx.x;
-    const int64_t seg = blockIdx.x % p.n_seg;
-    const int64_t bi = blockIdx.x / p.n_seg;
-
-    // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
-    float2 v[E];
-    {
-        const float2 *__restrict__ A = p.spectrum + bi * p.n_f;
-        const int64_t base = seg * p.S - p.m / 2;
-#pragma unroll
-        for (int d = 0; d < E; ++d) {
-            const int64_t k = base + d * NT + t;
-            v[d] = (k >= 0 && k < p.n_f) ? __ldg(A + k) : make_float2(0.f, 0.f);
-        }
-    }
-    // a2: forward FFT, once per segment (eq.(3))
-    fwd_from<C, 0>(v, buf0, buf1, p.tw, t);
-    float2 X[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) X[e] = v[e];
-    __syncthreads();
-
-    int bases[C::P];
-    fill_bases<C, 0>(bases, t);
-    InvTw<C> T;
-    load_inv_tw<C, 0>(T, p.tw, t);
-
-    // output geometry: register d of layout 0 holds y[d*NT + t]; kept if >= m; column = seg*S + p - m
-    const int64_t col0 = seg * p.S - p.m + t;                 // column of y[t]
-    float *__restrict__ prow = p.power + bi * p.n_z * p.n_f;  // row 0 of this batch item
-    const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
-    const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
-    const int d0 = p.m / NT;
-
-    const float4 *__restrict__ gp = p.gperm + t;
-    float4 g[E / 2];
-#pragma unroll
-    for (int q = 0; q < E / 2; ++q) g[q] = __ldg(gp + q * NT);
-
-    for (int z = 0; z < p.n_z; ++z) {
-        // a3: pointwise multiply by the transformed template ("convolution in the Fourier domain")
-#pragma unroll
-        for (int q = 0; q < E / 2; ++q) {
-            v[2 * q] = cmul(X[2 * q], make_float2(g[q].x, g[q].y));
-            v[2 * q + 1] = cmul(X[2 * q + 1], make_float2(g[q].z, g[q].w));
-        }
-        // prefetch the next template spectrum (L2 resident) while this one is transformed
-        if (z + 1 < p.n_z) {
-            gp += (E / 2) * NT;
-#pragma unroll
-            for (int q = 0; q < E / 2; ++q) g[q] = __ldg(gp + q * NT);
-        }
-        // a4: inverse FFT
-        butterflies<C, C::P - 1, true>(v);
-        inv_down<C, C::P - 2>(v, buf0, buf1, T, bases);
-        if constexpr ((C::P - 1) & 1) __syncthreads(); // odd number of exchanges: protect buffer reuse
-        // a5 + a6: trim, power, coalesced store
-        float *__restrict__ out = prow + (int64_t)z * p.n_f + col0;
-        if (fast) {
-#pragma unroll
-            for (int d = 0; d < E; ++d) {
-                if (d >= 4 || d >= d0) __stcs(out + d * NT, v[d].x * v[d].x + v[d].y * v[d].y);
-            }
-        } else {
-#pragma unroll
-            for (int d = 0; d < E; ++d) {
-                const int pidx = d * NT + t;
-                const int64_t col = col0 + d * NT;
-                if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = v[d].x * v[d].x + v[d].y * v[d].y;
-            }
-        }
-    }
-}
-
-// -------------------------------------------------------------------------------------------
-// Template preparation (off the hot path): G_z = DFT_L(pad(conj h_z)) / L in register order.
+// Template preparation (off the hot path): G_z = DFT_L(pad(conj h_z)) / L in the register order of
+// layout P-1 of the inverse transform, times the modulation exp(+2 pi i k NA a / Ra) that rotates
+// the outputs of the first inverse pass for the shuffle exchange (fft_device.cuh).
 // -------------------------------------------------------------------------------------------
 template <int L>
 __global__ void __launch_bounds__(Cfg<L>::NT) fdas_template_fft_kernel(const float2 *__restrict__ h, int m,
@@ -152,6 +31,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT) fdas_template_fft_kernel(const flo
                                                                        float4 *__restrict__ gperm)
 {
     using C = Cfg<L>;
+    using I = InvCfg<C>;
     constexpr int E = C::E, NT = C::NT;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x;
@@ -165,23 +45,30 @@ __global__ void __launch_bounds__(Cfg<L>::NT) fdas_template_fft_kernel(const flo
         if (j < m) { a = h[(size_t)z * m + j]; a.x *= scale; a.y *= -scale; } // conj(h) / L
         v[d] = a;
     }
-    fwd_from<C, 0>(v, smem, smem + C::SMEM_ELEMS, tw, t);
+    forward_to_inv_layout<C>(v, smem, smem + I::BUF_ELEMS, tw, t);
+#pragma unroll
+    for (int i = 0; i < I::NB; ++i)
+#pragma unroll
+        for (int k = 1; k < I::Ra; ++k) v[i * I::Ra + k] = cmulc(v[i * I::Ra + k], __ldg(tw + inv_gmod_index<C>(t, k)));
     float4 *g = gperm + (size_t)z * (E / 2) * NT + t;
 #pragma unroll
     for (int q = 0; q < E / 2; ++q) g[q * NT] = make_float4(v[2 * q].x, v[2 * q].y, v[2 * q + 1].x, v[2 * q + 1].y);
 }
 
 // -------------------------------------------------------------------------------------------
-// Debug FFT: natural order in, natural order out, either direction (tests only).
+// Debug FFT: natural order in, natural order out, either direction (tests only).  The inverse
+// runs the hot loop's inverse_transform and then removes the unit phase it leaves on each thread's
+// outputs (irrelevant to the power plane).
 // -------------------------------------------------------------------------------------------
 template <int L>
 __global__ void __launch_bounds__(Cfg<L>::NT) fdas_debug_fft_kernel(const float2 *__restrict__ in, float2 *__restrict__ out,
                                                                     const float2 *__restrict__ tw, int inverse)
 {
     using C = Cfg<L>;
+    using I = InvCfg<C>;
     constexpr int E = C::E, NT = C::NT, RL = C::R(C::P - 1), BL = E / RL;
     extern __shared__ float2 smem[];
-    float2 *buf0 = smem, *buf1 = smem + C::SMEM_ELEMS;
+    float2 *buf0 = smem, *buf1 = smem + I::BUF_ELEMS;
     const int t = threadIdx.x;
     const float2 *x = in + (size_t)blockIdx.x * L;
     float2 *y = out + (size_t)blockIdx.x * L;
@@ -189,7 +76,6 @@ __global__ void __launch_bounds__(Cfg<L>::NT) fdas_debug_fft_kernel(const float2
     if (!inverse) {
 #pragma unroll
         for (int d = 0; d < E; ++d) v[d] = x[d * NT + t];
-        __syncthreads();
         fwd_from<C, 0>(v, buf0, buf1, tw, t);
 #pragma unroll
         for (int b = 0; b < BL; ++b)
@@ -197,18 +83,20 @@ __global__ void __launch_bounds__(Cfg<L>::NT) fdas_debug_fft_kernel(const float2
             for (int d = 0; d < RL; ++d) y[nat_freq<C>(t, b, d)] = v[b * RL + d];
     } else {
 #pragma unroll
-        for (int b = 0; b < BL; ++b)
+        for (int i = 0; i < I::NB; ++i)
 #pragma unroll
-            for (int d = 0; d < RL; ++d) v[b * RL + d] = x[nat_freq<C>(t, b, d)];
-        __syncthreads();
-        int bases[C::P];
-        fill_bases<C, 0>(bases, t);
-        InvTw<C> T;
-        load_inv_tw<C, 0>(T, tw, t);
-        butterflies<C, C::P - 1, true>(v);
-        inv_down<C, C::P - 2>(v, buf0, buf1, T, bases);
+            for (int k = 0; k < I::Ra; ++k)
+                v[i * I::Ra + k] = cmulc(x[inv_freq<C>(t, i, k)], __ldg(tw + inv_gmod_index<C>(t, k)));
+        float2 tw0[C::R(0)];
+        tw0[0] = make_float2(1.f, 0.f);
 #pragma unroll
-        for (int d = 0; d < E; ++d) y[d * NT + t] = v[d];
+        for (int d = 1; d < C::R(0); ++d) tw0[d] = __ldg(tw + d * t);
+        const InvAddr<C> A = inv_addr<C>(t);
+        TwLdg<C> tws{tw, t};
+        inverse_transform<C>(v, buf0, buf1, A, tw0, tws, t & 31, []() {});
+        const float2 fix = __ldg(tw + inv_fix_index<C>(t));
+#pragma unroll
+        for (int d = 0; d < E; ++d) y[d * NT + t] = cmul(v[d], fix);
     }
 }
 
@@ -227,7 +115,6 @@ struct fdas_plan {
     float4 *d_gperm;   // n_z * L complex64
     float2 *d_tw;      // L complex64
     bool has_templates;
-    int variant;       // 2: TMEM-resident kernel (default); 1: register-resident kernel (FDAS_VARIANT=1)
     int last_cuda_error;
     int last_launches;
     // buffers of fdas_convolve_host
@@ -264,37 +151,21 @@ cudaError_t upload_twiddles(int L, float2 **d_tw)
     return e;
 }
 
-template <int L> size_t smem_bytes() { return 2 * sizeof(float2) * (size_t)Cfg<L>::SMEM_ELEMS; }
+template <int L> size_t smem_bytes() { return 2 * sizeof(float2) * (size_t)InvCfg<Cfg<L>>::BUF_ELEMS; }
 
-template <int L, int MINB> cudaError_t launch_convolve(const ConvParams &cp, int n_batch, cudaStream_t st)
+template <int L> cudaError_t launch_convolve(const ConvParams &cp, int n_batch, cudaStream_t st)
 {
-    auto kern = fdas_convolve_kernel<L, MINB>;
+    auto kern = fdas_convolve_kernel<L>;
+    constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
     static bool attr_done = false; // per instantiation; benign race (idempotent)
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<L>());
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     const int64_t blocks = cp.n_seg * n_batch;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    kern<<<(unsigned)blocks, Cfg<L>::NT, smem_bytes<L>(), st>>>(cp);
-    return cudaGetLastError();
-}
-
-template <int L> size_t smem_bytes_tmem() { return smem_bytes<L>() + sizeof(float2) * (size_t)L; }
-
-template <int L> cudaError_t launch_convolve_tmem(const ConvParams &cp, int n_batch, cudaStream_t st)
-{
-    auto kern = fdas_convolve_tmem_kernel<L>;
-    static bool attr_done = false; // per instantiation; benign race (idempotent)
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes_tmem<L>());
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
-    const int64_t blocks = cp.n_seg * n_batch;
-    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    kern<<<(unsigned)blocks, Cfg<L>::NT, smem_bytes_tmem<L>(), st>>>(cp);
+    kern<<<(unsigned)blocks, Cfg<L>::NT, smem, st>>>(cp);
     return cudaGetLastError();
 }
 
@@ -349,10 +220,6 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
     p->S = segment_len - template_width;
     p->n_seg = (n_f + p->S - 1) / p->S;
     p->n_batch = 1;
-    {
-        const char *v = getenv("FDAS_VARIANT");
-        p->variant = (v && v[0] == '1') ? 1 : 2;
-    }
     cudaError_t e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
     if (e == cudaSuccess) e = upload_twiddles(p->L, &p->d_tw);
     if (e != cudaSuccess) {
@@ -411,11 +278,7 @@ fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
-    if (p->variant == 1) {
-        FDAS_DISPATCH_L(L, (e = launch_convolve<LL, 1>(cp, p->n_batch, st)));
-    } else {
-        FDAS_DISPATCH_L(L, (e = launch_convolve_tmem<LL>(cp, p->n_batch, st)));
-    }
+    FDAS_DISPATCH_L(L, (e = launch_convolve<LL>(cp, p->n_batch, st)));
     p->last_launches = 1;
     if (e != cudaSuccess) return cuda_fail(p, e);
     return FDAS_OK;

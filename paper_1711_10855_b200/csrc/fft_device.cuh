@@ -171,4 +171,132 @@ template <class C, int I> __device__ __forceinline__ void fwd_from(float2 *v, fl
     }
 }
 
+
+// =============================================================================================
+// Inverse transform of the hot loop (a4): decimation in time, passes P-1 ... 0, where the exchange
+// between the first two passes is done with warp shuffles inside groups of Gs lanes and only the
+// remaining exchange(s) go through shared memory.
+//
+// Notation: Ra = R(P-1), Rb = R(P-2); a group of Gs = Ra*Rb/E consecutive threads owns the Ra*Rb
+// points that share the digits k_0..k_{P-3}; NB = E/Ra sub-transforms per thread in pass P-1,
+// NA = E/Rb in pass P-2.
+//   layout P-1  thread t = g*Gs + a, register i*Ra + k   <->  frequency digits (g; k_{P-2} = a*NB + i; k_{P-1} = k)
+//   layout P-2  thread t = g*Gs + c, register j*Rb + tau <->  (g; k_{P-2} = (s - tau) mod Rb; n_{P-1} = c*NA + j),
+//               s = NB*c + NB - 1
+// The transposition a <-> c needs lane-dependent register indices; they are made static by two
+// identities of the DFT:
+//   * rotating the OUTPUTS of pass P-1 by rho = NA*a is a modulation of its inputs by
+//     exp(+2 pi i k rho / Ra), which is folded into the template spectra G (per thread, off line);
+//   * presenting the INPUTS of pass P-2 reflected and rotated, x'[tau] = x[(s - tau) mod Rb], yields
+//     X'[kappa] = exp(2 pi i s kappa / Rb) X[-kappa]: a static index reflection and a unit phase
+//     that is constant over each later sub-transform and therefore vanishes in |.|^2.
+// In round r a thread sends registers {i*Ra + NA*r + j} to the lane r places up in its group and
+// receives into {j*Rb + NB*r + NB-1-i}: 2*(Gs-1)*NA*NB 32-bit shuffles, no barrier, no bank
+// conflicts, half the data-pipe wavefronts of a shared-memory exchange.
+// =============================================================================================
+template <class C> struct InvCfg {
+    static constexpr int P = C::P, E = C::E, NT = C::NT, L = C::L;
+    static constexpr int Ra = C::R(P - 1), Rb = C::R(P - 2);
+    static constexpr int Gs = Ra * Rb / E, NA = E / Rb, NB = E / Ra;
+    static constexpr int Q = Ra * Rb;                       // points per group
+    static constexpr int PAD = Gs >= 16 ? 0 : 8;            // half-warp = several groups: offset them by 8 banks
+    // P == 3: one exchange, element (k_0, n_1, n_2) at k_0*STR0 + n_1*Ra + n_2
+    // P == 4: exchange A, element (k_0, k_1, n_2, n_3) at (k_0*R1 + k_1)*STRX + n_2*Ra + n_3,
+    //         exchange B, element (k_0, n_1, n_2, n_3) at k_0*NT + n_1*Q + n_2*Ra + n_3
+    static constexpr int STR0 = (P == 3) ? NT + PAD : NT;
+    static constexpr int STRX = Q + PAD;
+    static constexpr int KK = NT / Q;                       // P == 4: values of k_0 per sub-transform slot
+    static constexpr int BUF_A = (P == 3) ? STR0 * C::R(0) : C::R(0) * C::R(1) * STRX;
+    static constexpr int BUF_B = (P == 3) ? STR0 * C::R(0) : L;
+    static constexpr int cmax(int a, int b) { return a > b ? a : b; }
+    static constexpr int BUF_ELEMS = cmax(cmax(BUF_A, BUF_B), cmax(C::SMEM_ELEMS, L)); // one of the two buffers
+    static_assert(P == 3 || P == 4, "three or four passes");
+    static_assert(Gs >= 2 && Gs <= 32 && (Gs & (Gs - 1)) == 0, "group must be a power of two within a warp");
+    static_assert(NA * Gs == Ra && NB * Gs == Rb, "group geometry");
+};
+
+// natural frequency index of register (i, k) of thread t in layout P-1 (new)
+template <class C> __device__ __forceinline__ int inv_freq(int t, int i, int k)
+{
+    using I = InvCfg<C>;
+    const int g = t / I::Gs, a = t % I::Gs;
+    const int kb = a * I::NB + i;
+    if constexpr (C::P == 3) return g + C::R(0) * (kb + C::R(1) * k);
+    else return (g / C::R(1)) + C::R(0) * ((g % C::R(1)) + C::R(1) * (kb + C::R(2) * k));
+}
+// index into w_L of the modulation folded into G: G' = G * conj(w_L^idx) = G * exp(+2 pi i k NA a / Ra)
+template <class C> __device__ __forceinline__ int inv_gmod_index(int t, int k)
+{
+    using I = InvCfg<C>;
+    return (k * I::NA * (t % I::Gs) * (C::L / I::Ra)) % C::L;
+}
+// index into w_L of the pass P-2 multiplier of register (j, tau): v *= conj(w_L^idx)
+template <class C> __device__ __forceinline__ int inv_twa_index(int t, int j, int tau)
+{
+    using I = InvCfg<C>;
+    const int c = t % I::Gs, s = I::NB * c + I::NB - 1, n = I::NA * c + j;
+    const int k_tau = ((s - tau) % I::Rb + I::Rb) % I::Rb, k_0 = s % I::Rb;
+    const int e = (k_tau - k_0) * n * (C::L / (I::Ra * I::Rb));
+    return ((e % C::L) + C::L) % C::L;
+}
+// index into w_L of the phase the outputs of thread t carry: true = out * w_L^idx ... (debug only)
+template <class C> __device__ __forceinline__ int inv_fix_index(int t)
+{
+    using I = InvCfg<C>;
+    const int q = t % I::Q, n_hi = q / I::Ra, n_lo = q % I::Ra;
+    const int c = n_lo / I::NA, kap = (I::Rb - n_hi) % I::Rb, s = I::NB * c + I::NB - 1;
+    // out * exp(-2 pi i s kap / Rb + 2 pi i (s mod Rb) n_lo / (Rb Ra)) = out * w_L^{s kap L/Rb - (s%Rb) n_lo L/(Ra Rb)}
+    const long long e = (long long)s * kap * (C::L / I::Rb) - (long long)(s % I::Rb) * n_lo * (C::L / (I::Ra * I::Rb));
+    return (int)(((e % C::L) + C::L) % C::L);
+}
+
+// the shuffle exchange: v in layout P-1 (pass P-1 done, outputs rotated), w in layout P-2
+template <class C> __device__ __forceinline__ void inv_shuffle(const float2 *v, float2 *w, int lane)
+{
+    using I = InvCfg<C>;
+#pragma unroll
+    for (int r = 0; r < I::Gs; ++r) {
+        const int src = lane + (I::Gs - r); // taken modulo the group width by the hardware
+#pragma unroll
+        for (int i = 0; i < I::NB; ++i)
+#pragma unroll
+            for (int j = 0; j < I::NA; ++j) {
+                float2 x = v[i * I::Ra + I::NA * r + j];
+                if (r) {
+                    x.x = __shfl_sync(0xffffffffu, x.x, src, I::Gs);
+                    x.y = __shfl_sync(0xffffffffu, x.y, src, I::Gs);
+                }
+                w[j * I::Rb + I::NB * r + I::NB - 1 - i] = x;
+            }
+    }
+}
+
+// shared-memory addresses of the remaining exchange(s)
+template <class C> struct InvAddr { int wa, ra, wb, rb; };
+template <class C> __device__ __forceinline__ InvAddr<C> inv_addr(int t)
+{
+    using I = InvCfg<C>;
+    InvAddr<C> A;
+    if constexpr (C::P == 3) {
+        A.wa = (t / I::Gs) * I::STR0 + I::NA * (t % I::Gs);
+        A.ra = t;
+        A.wb = A.rb = 0;
+    } else {
+        A.wa = (t / I::Gs) * I::STRX + I::NA * (t % I::Gs);
+        A.ra = (t / I::Q) * C::R(1) * I::STRX + (t % I::Q);
+        A.wb = (t / I::Q) * I::STR0 + (t % I::Q);
+        A.rb = t;
+    }
+    return A;
+}
+// write of layout P-2 registers (pass P-2 done): register j*Rb + kappa holds n_{P-2} = (-kappa) mod Rb
+template <class C> __device__ __forceinline__ void inv_write_a(float2 *buf, int wa, const float2 *w)
+{
+    using I = InvCfg<C>;
+#pragma unroll
+    for (int j = 0; j < I::NA; ++j)
+#pragma unroll
+        for (int kap = 0; kap < I::Rb; ++kap) buf[wa + ((I::Rb - kap) % I::Rb) * I::Ra + j] = w[j * I::Rb + kap];
+}
+
 } // namespace fdas
