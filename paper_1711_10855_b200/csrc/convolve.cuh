@@ -19,19 +19,27 @@
 namespace fdas {
 
 // ---------------------------------------------------------------------------------------------
-// inverse passes P-1 ... 0 on v (layout P-1, template already multiplied in).  TW supplies the
-// multipliers of pass P-2 (E entries, entry j*Rb is unused) and, for P == 4, of pass 1; tw0 holds
-// w_L^{d t} for pass 0.  All multipliers are applied conjugated (cmulc).  `hook` runs right after
-// the first block barrier.  P == 3: bufa alternates between calls (one barrier per call).
+// The inverse transform in three stages (passes P-1 ... 0; fft_device.cuh "Inverse transform of the
+// hot loop").  TW supplies the multipliers of pass P-2 (E entries, entry j*Rb is unused) and, for
+// P == 4, of pass 1; tw0 holds w_L^{d t} for pass 0.  All multipliers are applied conjugated.
+//   stage A  (in the caller) template multiply, then inv_stage_a: butterflies of pass P-1
+//   stage B  shuffle exchange, multipliers, butterflies of pass P-2, write to shared memory
+//   -- block barrier (the caller's: it may put independent work of the next z in front of it) --
+//   stage C  read, [P == 4: pass 1 and a second exchange with its own barrier,] pass 0
+// P == 3: bufa alternates between calls so that one barrier per transform suffices.
 // ---------------------------------------------------------------------------------------------
-template <class C, class TW, class Hook>
-__device__ __forceinline__ void inverse_transform(float2 *v, float2 *bufa, float2 *bufb, const InvAddr<C> &A, const float2 *tw0,
-                                                  TW &tws, int lane, Hook &&hook)
+template <class C> __device__ __forceinline__ void inv_stage_a(float2 *v)
+{
+    using I = InvCfg<C>;
+#pragma unroll
+    for (int i = 0; i < I::NB; ++i) Dft<I::Ra, true>::run(v + i * I::Ra);
+}
+
+template <class C, class TW>
+__device__ __forceinline__ void inv_stage_b(const float2 *v, float2 *bufa, const InvAddr<C> &A, TW &tws, int lane)
 {
     using I = InvCfg<C>;
     constexpr int E = C::E;
-#pragma unroll
-    for (int i = 0; i < I::NB; ++i) Dft<I::Ra, true>::run(v + i * I::Ra);
     float2 twa[E];
     tws.issue_a(twa);
     float2 w[E];
@@ -44,17 +52,22 @@ __device__ __forceinline__ void inverse_transform(float2 *v, float2 *bufa, float
 #pragma unroll
     for (int j = 0; j < I::NA; ++j) Dft<I::Rb, true>::run(w + j * I::Rb);
     inv_write_a<C>(bufa, A.wa, w);
+}
+
+template <class C, class TW>
+__device__ __forceinline__ void inv_stage_c(float2 *v, const float2 *bufa, float2 *bufb, const InvAddr<C> &A, const float2 *tw0, TW &tws)
+{
+    using I = InvCfg<C>;
+    constexpr int E = C::E;
+    float2 tw0t[C::R(0)];
+    if constexpr (TW::TW0_PARKED && C::P == 3) tws.issue_0(tw0t);
     if constexpr (C::P == 3) {
-        __syncthreads();
-        hook();
 #pragma unroll
         for (int k = 0; k < C::R(0); ++k) v[k] = bufa[A.ra + k * I::STR0];
     } else {
         constexpr int R1 = C::R(1), B1 = E / R1;
         float2 twm[8];
         tws.issue_m(twm);
-        __syncthreads();
-        hook();
 #pragma unroll
         for (int b = 0; b < B1; ++b)
 #pragma unroll
@@ -69,18 +82,26 @@ __device__ __forceinline__ void inverse_transform(float2 *v, float2 *bufa, float
 #pragma unroll
         for (int b = 0; b < B1; ++b)
 #pragma unroll
-            for (int n = 0; n < R1; ++n) bufb[A.wb + I::KK * b * I::STR0 + n * I::Q] = v[b * R1 + n];
+            for (int n = 0; n < R1; ++n) st_shared_f2(bufb + A.wb + I::KK * b * I::STR0 + n * I::Q, v[b * R1 + n]);
+        if constexpr (TW::TW0_PARKED) tws.issue_0(tw0t);
         __syncthreads();
 #pragma unroll
         for (int k = 0; k < C::R(0); ++k) v[k] = bufb[A.rb + k * I::STR0];
     }
+    if constexpr (TW::TW0_PARKED) {
+        tws.wait_0(tw0t);
 #pragma unroll
-    for (int d = 1; d < C::R(0); ++d) v[d] = cmulc(v[d], tw0[d]);
+        for (int d = 1; d < C::R(0); ++d) v[d] = cmulc(v[d], tw0t[d]);
+    } else {
+#pragma unroll
+        for (int d = 1; d < C::R(0); ++d) v[d] = cmulc(v[d], tw0[d]);
+    }
     Dft<C::R(0), true>::run(v);
 }
 
 // multipliers read from the w_L table in global memory (set-up code, debug kernel)
 template <class C> struct TwLdg {
+    static constexpr bool TW0_PARKED = false;
     const float2 *__restrict__ tw;
     int t;
     __device__ __forceinline__ void issue_a(float2 *o) const
@@ -109,18 +130,31 @@ template <class C> struct TwLdg {
 // tensor-memory geometry: per thread (TMEM lane) a block of columns X | TWA [| TWM]
 template <class C> struct TmemCfg {
     static constexpr int SLOTS = (C::NT + 127) / 128;          // warps sharing a 32-lane quarter
-    static constexpr int X_OFF = 0, TWA_OFF = 32, TWM_OFF = 64;
-    static constexpr int SLOT_COLS = C::P == 3 ? 64 : 128;
+    static constexpr int X_OFF = 0, TWA_OFF = 32, TW0_OFF = 64, TWM_OFF = 96;
+    static constexpr bool TW0_PARKED = C::NT >= 128;           // pass-0 multipliers in TMEM too (else registers)
+    static constexpr int SLOT_COLS = TW0_PARKED ? 128 : 64;
     static constexpr int NCOLS_RAW = SLOT_COLS * SLOTS;
     static constexpr int NCOLS = NCOLS_RAW <= 32 ? 32 : NCOLS_RAW <= 64 ? 64 : NCOLS_RAW <= 128 ? 128 : NCOLS_RAW <= 256 ? 256 : 512;
     static constexpr int MINB = (512 / C::NT) > 0 ? (512 / C::NT) : 1; // CTAs per SM at 128 registers
     static_assert(2 * C::E <= 32, "a segment slice or a twiddle block is at most 32 columns");
     static_assert(NCOLS_RAW <= 512 && NCOLS * MINB <= 512, "tensor memory holds 512 columns per SM");
+    static_assert(TW0_PARKED || C::P == 3, "four passes need the 128-column block");
 };
 
 // multipliers parked in tensor memory
 template <class C> struct TwTmem {
+    static constexpr bool TW0_PARKED = TmemCfg<C>::TW0_PARKED;
     uint32_t addr; // TMEM address of this thread's column block
+    __device__ __forceinline__ void issue_0(float2 *o) const
+    {
+        ptx::tmem_ld16(addr + TmemCfg<C>::TW0_OFF, o);
+        if constexpr (C::R(0) > 8) ptx::tmem_ld16(addr + TmemCfg<C>::TW0_OFF + 16, o + 8);
+    }
+    __device__ __forceinline__ void wait_0(float2 *o) const
+    {
+        ptx::tmem_wait_ld8(o);
+        if constexpr (C::R(0) > 8) ptx::tmem_wait_ld8(o + 8);
+    }
     __device__ __forceinline__ void issue_a(float2 *o) const
     {
         ptx::tmem_ld16(addr + TmemCfg<C>::TWA_OFF, o);
@@ -228,11 +262,19 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     if constexpr (E > 8) ptx::tmem_st16(tm_addr + TC::X_OFF + 16, v + 8);
 
     // inverse multipliers (independent of z): pass 0 in registers, the others in tensor memory
-    float2 tw0[C::R(0)];
+    float2 tw0[TC::TW0_PARKED ? 1 : C::R(0)];
     {
-        tw0[0] = make_float2(1.f, 0.f);
+        if constexpr (TC::TW0_PARKED) {
+            float2 w0[16];
 #pragma unroll
-        for (int d = 1; d < C::R(0); ++d) tw0[d] = __ldg(p.tw + d * t);
+            for (int d = 0; d < 16; ++d) w0[d] = (d && d < C::R(0)) ? __ldg(p.tw + d * t) : make_float2(1.f, 0.f);
+            ptx::tmem_st16(tm_addr + TC::TW0_OFF, w0);
+            if constexpr (C::R(0) > 8) ptx::tmem_st16(tm_addr + TC::TW0_OFF + 16, w0 + 8);
+        } else {
+            tw0[0] = make_float2(1.f, 0.f);
+#pragma unroll
+            for (int d = 1; d < C::R(0); ++d) tw0[d] = __ldg(p.tw + d * t);
+        }
         TwLdg<C> src{p.tw, t};
         float2 w[16];
 #pragma unroll
@@ -246,7 +288,6 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
         }
     }
     ptx::tmem_wait_st();
-    __syncthreads(); // the forward transform's last reads of buf0 are done before the z loop writes it
 
     const InvAddr<C> A = inv_addr<C>(t);
     TwTmem<C> tws{tm_addr};
@@ -257,8 +298,9 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
     const int d0 = p.m / NT;
 
-    for (int z = 0; z < p.n_z; ++z) {
-        // a3: pointwise multiply by the transformed template ("convolution in the Fourier domain")
+    // a3 + first inverse pass of template z ("convolution in the Fourier domain"; "for every
+    // matched filter"): v = X * G_z in layout P-1, butterflies of pass P-1
+    auto stage_a = [&](int z) {
         float2 X[E];
         ptx::tmem_ld16(tm_addr + TC::X_OFF, X);
         if constexpr (E > 8) ptx::tmem_ld16(tm_addr + TC::X_OFF + 16, X + 8);
@@ -271,28 +313,42 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
             v[2 * q] = cmul(X[2 * q], make_float2(g.x, g.y));
             v[2 * q + 1] = cmul(X[2 * q + 1], make_float2(g.z, g.w));
         }
-        // a4: inverse FFT.  After its first block barrier every thread has consumed G_z, so the
-        // elected thread starts the bulk copy of G_{z+1} into the same stage.
+        inv_stage_a<C>(v);
+    };
+    auto fetch_g = [&](int z) { // elected thread: bulk copy of G_z into the stage (every thread is past its reads)
+        if (t == 0 && z < p.n_z) {
+            ptx::mbar_expect_tx(&g_bar, G_BYTES);
+            ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)z * G_BYTES, G_BYTES, &g_bar);
+        }
+    };
+    stage_a(0);
+    __syncthreads(); // also: the forward transform's last reads of buf0 are done before the z loop writes it
+    fetch_g(1);
+
+    // The z loop is software pipelined: stage A of template z+1 (tensor-memory and shared-memory
+    // reads, 1/3 of the arithmetic) sits between the exchange write of template z and its barrier, so
+    // a warp that reaches the barrier early has independent work instead of idling.
+    for (int z = 0; z < p.n_z; ++z) {
         float2 *bufa = (C::P == 3 && (z & 1)) ? buf1 : buf0;
-        inverse_transform<C>(v, bufa, buf1, A, tw0, tws, lane, [&]() {
-            if (t == 0 && z + 1 < p.n_z) {
-                ptx::mbar_expect_tx(&g_bar, G_BYTES);
-                ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)(z + 1) * G_BYTES, G_BYTES, &g_bar);
-            }
-        });
+        inv_stage_b<C>(v, bufa, A, tws, lane);
+        if (z + 1 < p.n_z) stage_a(z + 1);
+        __syncthreads();
+        fetch_g(z + 2);
+        float2 u[E];
+        inv_stage_c<C>(u, bufa, buf1, A, tw0, tws);
         // a5 + a6: trim, power, coalesced store
         float *__restrict__ out = prow + (int64_t)z * p.n_f + col0;
         if (fast) {
 #pragma unroll
             for (int d = 0; d < E; ++d) {
-                if (d >= 4 || d >= d0) __stcs(out + d * NT, v[d].x * v[d].x + v[d].y * v[d].y);
+                if (d >= 4 || d >= d0) __stcs(out + d * NT, u[d].x * u[d].x + u[d].y * u[d].y);
             }
         } else {
 #pragma unroll
             for (int d = 0; d < E; ++d) {
                 const int pidx = d * NT + t;
                 const int64_t col = col0 + d * NT;
-                if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = v[d].x * v[d].x + v[d].y * v[d].y;
+                if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = u[d].x * u[d].x + u[d].y * u[d].y;
             }
         }
     }

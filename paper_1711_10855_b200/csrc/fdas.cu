@@ -93,7 +93,10 @@ __global__ void __launch_bounds__(Cfg<L>::NT) fdas_debug_fft_kernel(const float2
         for (int d = 1; d < C::R(0); ++d) tw0[d] = __ldg(tw + d * t);
         const InvAddr<C> A = inv_addr<C>(t);
         TwLdg<C> tws{tw, t};
-        inverse_transform<C>(v, buf0, buf1, A, tw0, tws, t & 31, []() {});
+        inv_stage_a<C>(v);
+        inv_stage_b<C>(v, buf0, A, tws, t & 31);
+        __syncthreads();
+        inv_stage_c<C>(v, buf0, buf1, A, tw0, tws);
         const float2 fix = __ldg(tw + inv_fix_index<C>(t));
 #pragma unroll
         for (int d = 0; d < E; ++d) y[d * NT + t] = cmul(v[d], fix);

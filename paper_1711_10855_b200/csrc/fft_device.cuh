@@ -250,6 +250,14 @@ template <class C> __device__ __forceinline__ int inv_fix_index(int t)
     return (int)(((e % C::L) + C::L) % C::L);
 }
 
+// 64-bit shared-memory store written as PTX so that the data operands are the producing
+// instruction's own register pair (the C++ struct copy made ptxas stage every store through one
+// scratch pair, a MOV/MOV/STS chain serialised by the store's read scoreboard).
+__device__ __forceinline__ void st_shared_f2(float2 *p, float2 v)
+{
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"((unsigned)__cvta_generic_to_shared(p)), "f"(v.x), "f"(v.y) : "memory");
+}
+
 // the shuffle exchange: v in layout P-1 (pass P-1 done, outputs rotated), w in layout P-2
 template <class C> __device__ __forceinline__ void inv_shuffle(const float2 *v, float2 *w, int lane)
 {
@@ -296,7 +304,7 @@ template <class C> __device__ __forceinline__ void inv_write_a(float2 *buf, int 
 #pragma unroll
     for (int j = 0; j < I::NA; ++j)
 #pragma unroll
-        for (int kap = 0; kap < I::Rb; ++kap) buf[wa + ((I::Rb - kap) % I::Rb) * I::Ra + j] = w[j * I::Rb + kap];
+        for (int kap = 0; kap < I::Rb; ++kap) st_shared_f2(buf + wa + ((I::Rb - kap) % I::Rb) * I::Ra + j, w[j * I::Rb + kap]);
 }
 
 } // namespace fdas
