@@ -125,6 +125,22 @@ class ClockSampler:
                 "power_w": float(np.median(pw)) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(value, world, device=None):
+    """MAX over ranks of a per-rank scalar (device time in ms); no data-path collective exists on this
+    path, this is the timing reduction only.  Works on NCCL (GPU tensor) and gloo (CPU tensor)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(points_per_rank, world, steps, total_ms_max):
+    """(z,r) points all ranks processed over the slowest rank's device time (weak scaling)."""
+    return world * points_per_rank * steps / (total_ms_max * 1e-3)
+
+
 def make_workload(args, rank):
     from paper_1711_10855_b200 import workload
     c = args.config
@@ -249,12 +265,9 @@ def run_ours(args):
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     total_ms = ev[0].elapsed_time(ev[-1])
     per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
+    total_ms_max = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms_max / args.steps
-    value = world * points * args.steps / (total_ms_max * 1e-3)
+    value = whole_job_value(points, world, args.steps, total_ms_max)
 
     # e2e: host buffers through the C ABI, copies inside the timed region
     e2e = None
@@ -270,12 +283,10 @@ def run_ours(args):
             plan.convolve_host(h_spec, h_pow, stream=stream)
         e1.record(stream)
         barrier()
-        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * points * e2e_steps / (float(te.item()) * 1e-3), "unit": UNIT,
+        te = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+        e2e = {"value": whole_job_value(points, world, e2e_steps, te), "unit": UNIT,
                "h2d_bytes_per_step": int(h_spec.numel() * 8), "d2h_bytes_per_step": int(h_pow.numel() * 4),
-               "steps": e2e_steps, "ms_per_step": float(te.item()) / e2e_steps}
+               "steps": e2e_steps, "ms_per_step": te / e2e_steps}
         del h_pow
 
     if rank == 0:
@@ -295,7 +306,7 @@ def run_ours(args):
             "unit": "TFLOP/s" if alu_binds else "GB/s",
             "frac": (ach_tf / fp32_peak) if alu_binds else (ach_gb / pk["hbm_gbs"]),
             "traffic": traffic[0], "traffic_source": traffic[1],
-            "kernel": f"fdas_convolve_kernel<{wl.seg_len}>", "kernel_ms": kern_ms, "kernel_ms_min": float(np.min(per_launch_ms)),
+            "kernel": f"fdas::fdas_convolve_kernel<{wl.seg_len}>", "kernel_ms": kern_ms, "kernel_ms_min": float(np.min(per_launch_ms)),
             "flops_per_launch": flops_alg, "bytes_per_launch": bytes_alg,
             "alu": {"achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach_tf / fp32_peak,
                     "peak_def": f"{N_SM} SMs x {FP32_LANES_PER_SM} lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (nominal; flops = 5 L log2 L per transform)"},

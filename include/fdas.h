@@ -127,6 +127,32 @@ const char *fdas_status_string(fdas_status s);
  */
 fdas_status fdas_debug_fft(int segment_len, int64_t n_seg, const void *d_in, void *d_out, int inverse);
 
+/*
+ * Debug / test entry (HOST only, no GPU needed): evaluates the index maps of the inverse transform
+ * of the hot loop exactly as the kernels do (same functions, compiled for the host), so that the
+ * layout logic -- which element a thread register holds, the shuffle register permutation, the
+ * shared-memory addresses of the exchanges and the twiddle-table indices -- can be checked on a CPU.
+ *   what = FDAS_LAYOUT_GEOMETRY  a selects: 0 P (passes), 1 E (elements/thread), 2 NT (threads),
+ *          3 Ra, 4 Rb (radices of the first two inverse passes), 5 Gs (shuffle group), 6 NA, 7 NB,
+ *          8 elements of one exchange buffer, 9 R0, 10 R1
+ *   FDAS_LAYOUT_FREQ      natural frequency index held by register a*Ra + b of thread t at loop entry
+ *   FDAS_LAYOUT_GMOD      index j: the template spectrum element of register (., a) is stored times conj(w_L^j)
+ *   FDAS_LAYOUT_TWA       index j: register a*Rb + b is multiplied by conj(w_L^j) before the second pass
+ *   FDAS_LAYOUT_FIX       index j: thread t's outputs equal the exact inverse DFT times conj(w_L^j)
+ *   FDAS_LAYOUT_SHFL_SRC / _DST  register sent / written in shuffle round a for the pair b = i*NA + j
+ *   FDAS_LAYOUT_WRITE_A   shared-memory element written from register a*Rb + b (first exchange)
+ *   FDAS_LAYOUT_READ_A    shared-memory element read into register a*R + b   (R = R0 if P == 3, else R1)
+ *   FDAS_LAYOUT_WRITE_B / _READ_B  second exchange (P == 4 only): register a*R1 + b / register a
+ *   FDAS_LAYOUT_TW_MID    (P == 4) index j: register (., a) of the third pass is multiplied by conj(w_L^j)
+ * w_L = exp(-2 pi i / L).  Returns -1 for arguments out of range or an unsupported segment_len.
+ */
+enum {
+    FDAS_LAYOUT_GEOMETRY = 0, FDAS_LAYOUT_FREQ = 1, FDAS_LAYOUT_GMOD = 2, FDAS_LAYOUT_TWA = 3, FDAS_LAYOUT_FIX = 4,
+    FDAS_LAYOUT_SHFL_SRC = 5, FDAS_LAYOUT_SHFL_DST = 6, FDAS_LAYOUT_WRITE_A = 7, FDAS_LAYOUT_READ_A = 8,
+    FDAS_LAYOUT_WRITE_B = 9, FDAS_LAYOUT_READ_B = 10, FDAS_LAYOUT_TW_MID = 11
+};
+int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b);
+
 /* Library build info: e.g. "libfdas sm_100a <date>".  Never NULL. */
 const char *fdas_version(void);
 

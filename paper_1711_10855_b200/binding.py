@@ -31,6 +31,7 @@ SYMBOLS = {
     "fdas_plan_last_cuda_error": (_int, [_vp]),
     "fdas_status_string": (ctypes.c_char_p, [_int]),
     "fdas_debug_fft": (_int, [_int, _i64, _vp, _vp, _int]),
+    "fdas_debug_layout": (_i64, [_int, _int, _int, _int, _int]),
     "fdas_version": (ctypes.c_char_p, []),
 }
 
@@ -151,3 +152,13 @@ class Plan:
 def debug_fft(segment_len, n_seg, d_in, d_out, inverse=False):
     _check(lib().fdas_debug_fft(int(segment_len), int(n_seg), _ptr(d_in), _ptr(d_out), int(bool(inverse))),
            "fdas_debug_fft")
+
+
+# `what` selectors of fdas_debug_layout (include/fdas.h)
+(LAYOUT_GEOMETRY, LAYOUT_FREQ, LAYOUT_GMOD, LAYOUT_TWA, LAYOUT_FIX, LAYOUT_SHFL_SRC, LAYOUT_SHFL_DST,
+ LAYOUT_WRITE_A, LAYOUT_READ_A, LAYOUT_WRITE_B, LAYOUT_READ_B, LAYOUT_TW_MID) = range(12)
+
+
+def debug_layout(segment_len, what, t=0, a=0, b=0) -> int:
+    """Host evaluation of the kernels' index maps (no GPU needed); -1 = out of range."""
+    return int(lib().fdas_debug_layout(int(segment_len), int(what), int(t), int(a), int(b)))

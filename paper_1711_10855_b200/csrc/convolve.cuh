@@ -63,7 +63,7 @@ __device__ __forceinline__ void inv_stage_c(float2 *v, const float2 *bufa, float
     if constexpr (TW::TW0_PARKED && C::P == 3) tws.issue_0(tw0t);
     if constexpr (C::P == 3) {
 #pragma unroll
-        for (int k = 0; k < C::R(0); ++k) v[k] = bufa[A.ra + k * I::STR0];
+        for (int k = 0; k < C::R(0); ++k) v[k] = bufa[A.ra + I::ra_off(0, k)];
     } else {
         constexpr int R1 = C::R(1), B1 = E / R1;
         float2 twm[8];
@@ -71,7 +71,7 @@ __device__ __forceinline__ void inv_stage_c(float2 *v, const float2 *bufa, float
 #pragma unroll
         for (int b = 0; b < B1; ++b)
 #pragma unroll
-            for (int k = 0; k < R1; ++k) v[b * R1 + k] = bufa[A.ra + (b * I::KK * R1 + k) * I::STRX];
+            for (int k = 0; k < R1; ++k) v[b * R1 + k] = bufa[A.ra + I::ra_off(b, k)];
         tws.wait_m(twm);
 #pragma unroll
         for (int d = 1; d < R1; ++d)
@@ -82,11 +82,11 @@ __device__ __forceinline__ void inv_stage_c(float2 *v, const float2 *bufa, float
 #pragma unroll
         for (int b = 0; b < B1; ++b)
 #pragma unroll
-            for (int n = 0; n < R1; ++n) st_shared_f2(bufb + A.wb + I::KK * b * I::STR0 + n * I::Q, v[b * R1 + n]);
+            for (int n = 0; n < R1; ++n) st_shared_f2(bufb + A.wb + I::wb_off(b, n), v[b * R1 + n]);
         if constexpr (TW::TW0_PARKED) tws.issue_0(tw0t);
         __syncthreads();
 #pragma unroll
-        for (int k = 0; k < C::R(0); ++k) v[k] = bufb[A.rb + k * I::STR0];
+        for (int k = 0; k < C::R(0); ++k) v[k] = bufb[A.rb + I::rb_off(k)];
     }
     if constexpr (TW::TW0_PARKED) {
         tws.wait_0(tw0t);

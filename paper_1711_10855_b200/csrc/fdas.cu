@@ -3,8 +3,9 @@
 // arXiv:1711.10855 (P:NN = PAPER.md line NN): eq.(2) P:23 evaluated by overlap-and-save with
 // an on-chip FFT (eq.(3)) that is called once forward per segment and once inverse
 // per matched filter ("called for every matched filter").  One CTA owns one segment: the
-// forward-transformed segment stays in REGISTERS across all n_z templates, so the spectrum is read
-// from HBM once per segment and the only HBM stream of the z loop is the coalesced power-plane write.
+// forward-transformed segment stays ON CHIP (tensor memory) across all n_z templates, so the spectrum
+// is read from HBM once per segment and the only HBM stream of the z loop is the coalesced power-plane
+// write.  The kernels are in convolve.cuh / fft_device.cuh; this file holds the C ABI.
 //
 // Built for sm_100a only.  No cuFFT, no CPU fallback.
 #include <cuda_runtime.h>
@@ -202,6 +203,44 @@ template <int L> cudaError_t launch_debug_fft(int64_t n_seg, const float2 *in, f
 
 } // namespace
 
+// Host evaluation of the index maps the kernels use (fft_device.cuh): for tests without a GPU.
+template <int L> static int64_t layout_query(int what, int t, int a, int b)
+{
+    using C = Cfg<L>;
+    using I = InvCfg<C>;
+    if (t < 0 || t >= C::NT) return -1;
+    const InvAddr<C> A = inv_addr<C>(t);
+    switch (what) {
+    case FDAS_LAYOUT_GEOMETRY:
+        switch (a) {
+        case 0: return C::P;
+        case 1: return C::E;
+        case 2: return C::NT;
+        case 3: return I::Ra;
+        case 4: return I::Rb;
+        case 5: return I::Gs;
+        case 6: return I::NA;
+        case 7: return I::NB;
+        case 8: return I::BUF_ELEMS;
+        case 9: return C::R(0);
+        case 10: return C::R(1);
+        default: return -1;
+        }
+    case FDAS_LAYOUT_FREQ: return inv_freq<C>(t, a, b);
+    case FDAS_LAYOUT_GMOD: return inv_gmod_index<C>(t, a);
+    case FDAS_LAYOUT_TWA: return inv_twa_index<C>(t, a, b);
+    case FDAS_LAYOUT_FIX: return inv_fix_index<C>(t);
+    case FDAS_LAYOUT_SHFL_SRC: return I::shfl_src_reg(a, b / I::NA, b % I::NA);
+    case FDAS_LAYOUT_SHFL_DST: return I::shfl_dst_reg(a, b / I::NA, b % I::NA);
+    case FDAS_LAYOUT_WRITE_A: return A.wa + I::wa_off(a, b);
+    case FDAS_LAYOUT_READ_A: return A.ra + I::ra_off(a, b);
+    case FDAS_LAYOUT_WRITE_B: return C::P == 4 ? A.wb + I::wb_off(a, b) : -1;
+    case FDAS_LAYOUT_READ_B: return C::P == 4 ? A.rb + I::rb_off(a) : -1;
+    case FDAS_LAYOUT_TW_MID: return C::P == 4 ? a * ((t % C::Lo(1)) * (C::L / (C::R(1) * C::Lo(1)))) : -1;
+    default: return -1;
+    }
+}
+
 extern "C" {
 
 fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step, int template_width, int segment_len)
@@ -365,6 +404,13 @@ fdas_status fdas_debug_fft(int segment_len, int64_t n_seg, const void *d_in, voi
     if (d_tw) cudaFree(d_tw);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
     return FDAS_OK;
+}
+
+int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b)
+{
+    int64_t r = -1;
+    FDAS_DISPATCH_L(segment_len, r = layout_query<LL>(what, t, a, b));
+    return r;
 }
 
 const char *fdas_version(void) { return "libfdas sm_100a " __DATE__; }

@@ -210,13 +210,21 @@ template <class C> struct InvCfg {
     static constexpr int BUF_B = (P == 3) ? STR0 * C::R(0) : L;
     static constexpr int cmax(int a, int b) { return a > b ? a : b; }
     static constexpr int BUF_ELEMS = cmax(cmax(BUF_A, BUF_B), cmax(C::SMEM_ELEMS, L)); // one of the two buffers
+    // register maps of the shuffle exchange (round r, sub-transforms i of pass P-1 and j of pass P-2)
+    __host__ __device__ static constexpr int shfl_src_reg(int r, int i, int j) { return i * Ra + NA * r + j; }
+    __host__ __device__ static constexpr int shfl_dst_reg(int r, int i, int j) { return j * Rb + NB * r + NB - 1 - i; }
+    // shared-memory offsets relative to InvAddr (complex elements)
+    __host__ __device__ static constexpr int wa_off(int j, int kap) { return ((Rb - kap) % Rb) * Ra + j; } // register j*Rb+kap
+    __host__ __device__ static constexpr int ra_off(int b, int k) { return P == 3 ? k * STR0 : (b * KK * C::R(1) + k) * STRX; }
+    __host__ __device__ static constexpr int wb_off(int b, int n) { return KK * b * STR0 + n * Q; }         // P == 4 only
+    __host__ __device__ static constexpr int rb_off(int k) { return k * STR0; }                             // P == 4 only
     static_assert(P == 3 || P == 4, "three or four passes");
     static_assert(Gs >= 2 && Gs <= 32 && (Gs & (Gs - 1)) == 0, "group must be a power of two within a warp");
     static_assert(NA * Gs == Ra && NB * Gs == Rb, "group geometry");
 };
 
 // natural frequency index of register (i, k) of thread t in layout P-1 (new)
-template <class C> __device__ __forceinline__ int inv_freq(int t, int i, int k)
+template <class C> __host__ __device__ __forceinline__ int inv_freq(int t, int i, int k)
 {
     using I = InvCfg<C>;
     const int g = t / I::Gs, a = t % I::Gs;
@@ -225,13 +233,13 @@ template <class C> __device__ __forceinline__ int inv_freq(int t, int i, int k)
     else return (g / C::R(1)) + C::R(0) * ((g % C::R(1)) + C::R(1) * (kb + C::R(2) * k));
 }
 // index into w_L of the modulation folded into G: G' = G * conj(w_L^idx) = G * exp(+2 pi i k NA a / Ra)
-template <class C> __device__ __forceinline__ int inv_gmod_index(int t, int k)
+template <class C> __host__ __device__ __forceinline__ int inv_gmod_index(int t, int k)
 {
     using I = InvCfg<C>;
     return (k * I::NA * (t % I::Gs) * (C::L / I::Ra)) % C::L;
 }
 // index into w_L of the pass P-2 multiplier of register (j, tau): v *= conj(w_L^idx)
-template <class C> __device__ __forceinline__ int inv_twa_index(int t, int j, int tau)
+template <class C> __host__ __device__ __forceinline__ int inv_twa_index(int t, int j, int tau)
 {
     using I = InvCfg<C>;
     const int c = t % I::Gs, s = I::NB * c + I::NB - 1, n = I::NA * c + j;
@@ -240,7 +248,7 @@ template <class C> __device__ __forceinline__ int inv_twa_index(int t, int j, in
     return ((e % C::L) + C::L) % C::L;
 }
 // index into w_L of the phase the outputs of thread t carry: true = out * w_L^idx ... (debug only)
-template <class C> __device__ __forceinline__ int inv_fix_index(int t)
+template <class C> __host__ __device__ __forceinline__ int inv_fix_index(int t)
 {
     using I = InvCfg<C>;
     const int q = t % I::Q, n_hi = q / I::Ra, n_lo = q % I::Ra;
@@ -269,19 +277,19 @@ template <class C> __device__ __forceinline__ void inv_shuffle(const float2 *v, 
         for (int i = 0; i < I::NB; ++i)
 #pragma unroll
             for (int j = 0; j < I::NA; ++j) {
-                float2 x = v[i * I::Ra + I::NA * r + j];
+                float2 x = v[I::shfl_src_reg(r, i, j)];
                 if (r) {
                     x.x = __shfl_sync(0xffffffffu, x.x, src, I::Gs);
                     x.y = __shfl_sync(0xffffffffu, x.y, src, I::Gs);
                 }
-                w[j * I::Rb + I::NB * r + I::NB - 1 - i] = x;
+                w[I::shfl_dst_reg(r, i, j)] = x;
             }
     }
 }
 
 // shared-memory addresses of the remaining exchange(s)
 template <class C> struct InvAddr { int wa, ra, wb, rb; };
-template <class C> __device__ __forceinline__ InvAddr<C> inv_addr(int t)
+template <class C> __host__ __device__ __forceinline__ InvAddr<C> inv_addr(int t)
 {
     using I = InvCfg<C>;
     InvAddr<C> A;
@@ -304,7 +312,7 @@ template <class C> __device__ __forceinline__ void inv_write_a(float2 *buf, int 
 #pragma unroll
     for (int j = 0; j < I::NA; ++j)
 #pragma unroll
-        for (int kap = 0; kap < I::Rb; ++kap) st_shared_f2(buf + wa + ((I::Rb - kap) % I::Rb) * I::Ra + j, w[j * I::Rb + kap]);
+        for (int kap = 0; kap < I::Rb; ++kap) st_shared_f2(buf + wa + I::wa_off(j, kap), w[j * I::Rb + kap]);
 }
 
 } // namespace fdas
