@@ -209,3 +209,40 @@ def test_convolve_host_equals_device(torch, binding):
     plan.convolve_host(h_spec, h_pow)
     assert torch.equal(h_pow, d_pow.cpu())
     plan.destroy()
+
+
+@pytest.mark.parametrize("L,m", [(512, 64), (1024, 128), (2048, 256), (4096, 512), (8192, 1024)])
+def test_repeated_launches_are_bitwise_identical(torch, binding, L, m):
+    """Race detector of last resort (compute-sanitizer is not available on the GPU pool): the hot loop
+    re-uses its exchange buffers, template stage and tensor memory across z with one barrier per exchange;
+    a missing ordering shows up as run-to-run differences.  Many CTAs per SM, several launches, two streams,
+    every segment length; and the first launch is checked against an independent single-segment plan."""
+    n_f = 40 * (L - m) + 17
+    H = workload.templates(40, 2, m).astype(np.complex64)
+    spec = workload.noise_spectrum(n_f, 99 + L, 3)
+    plan = binding.Plan(n_f, 40, 2, m, L, n_batch=3)
+    plan.set_templates(H)
+    d_spec = torch.from_numpy(spec).cuda()
+    outs = [torch.full((3, 41, n_f), float("nan"), dtype=torch.float32, device="cuda") for _ in range(6)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for i, o in enumerate(outs):
+        plan.convolve(d_spec, o, stream=streams[i % 2])
+    torch.cuda.synchronize()
+    for o in outs[1:]:
+        assert torch.equal(outs[0], o)
+    assert bool(torch.isfinite(outs[0]).all())
+    # the same columns from a plan that sees only a window of the spectrum (different CTA <-> segment map)
+    c0, c1 = 7 * (L - m), 9 * (L - m)
+    lo, hi = c0 - m, c1 + m
+    sub = binding.Plan(hi - lo, 40, 2, m, L, n_batch=1)
+    sub.set_templates(H)
+    d_sub = torch.from_numpy(np.ascontiguousarray(spec[1:2, lo:hi])).cuda()
+    o_sub = torch.empty((1, 41, hi - lo), dtype=torch.float32, device="cuda")
+    sub.convolve(d_sub, o_sub)
+    torch.cuda.synchronize()
+    a = outs[0][1, :, c0:c1].cpu().numpy().astype(np.float64)
+    b = o_sub[0, :, c0 - lo:c1 - lo].cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(a - b)) <= 1e-5 * a.max()
+    plan.destroy()
+    sub.destroy()
