@@ -8,10 +8,12 @@
 //     registers nor LSU / shared-memory bandwidth;
 //   * G_z is brought from L2 into shared memory by the bulk-copy engine (cp.async.bulk, one elected
 //     thread, mbarrier completion) one z ahead and read with conflict-free LDS.128;
-//   * the working set v, the pass-0 twiddles and addressing stay in registers (<= 128 registers, two
-//     256-thread CTAs per SM at L = 4096).
+//   * only the working set v and addressing stay in registers (<= 128 registers, two 256-thread CTAs
+//     per SM at L = 4096; the 64-thread plans L = 512, 1024 keep the pass-0 twiddles in registers too).
 // The inverse transform (fft_device.cuh, "Inverse transform of the hot loop") exchanges data once
 // by warp shuffles and once (L = 8192: twice) through shared memory; one barrier per exchange.
+// The z loop is software pipelined: stage A of template z+1 runs before the barrier of template z.
+// Measured cost model, ablations and the experiments that did not help: profiles/r1_c3_v4.md.
 #pragma once
 #include "fft_device.cuh"
 #include "sm100_ptx.cuh"
