@@ -161,16 +161,17 @@ template <int L> cudaError_t launch_convolve(const ConvParams &cp, int n_batch, 
 {
     auto kern = fdas_convolve_kernel<L>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
-    static bool attr_done = false; // per instantiation; benign race (idempotent)
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
     const int64_t blocks = cp.n_seg * n_batch;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     kern<<<(unsigned)blocks, Cfg<L>::NT, smem, st>>>(cp);
     return cudaGetLastError();
+}
+
+// opt the hot kernel of this segment length in to its dynamic shared memory (once per plan, at creation)
+template <int L> cudaError_t prepare_convolve()
+{
+    return cudaFuncSetAttribute(fdas_convolve_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)conv_smem_bytes<Cfg<L>>());
 }
 
 template <int L> cudaError_t launch_template_fft(const float2 *d_h, int m, int n_z, const float2 *d_tw, float4 *d_g)
@@ -264,6 +265,10 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
     p->n_batch = 1;
     cudaError_t e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
     if (e == cudaSuccess) e = upload_twiddles(p->L, &p->d_tw);
+    if (e == cudaSuccess) {
+        const int L = p->L;
+        FDAS_DISPATCH_L(L, e = prepare_convolve<LL>());
+    }
     if (e != cudaSuccess) {
         fdas_status s = (e == cudaErrorMemoryAllocation) ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
         (void)cudaGetLastError();
