@@ -10,6 +10,10 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box via gpurun)")
+    # a fresh checkout has no libfdas.so (built artefacts are git-ignored): build it once, in tree, with
+    # nvcc for sm_100a (cross-compiles without a GPU).  The library itself never builds or falls back.
+    from paper_1711_10855_b200 import build as _build
+    _build.build()
 
 
 @pytest.fixture(scope="session")
