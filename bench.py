@@ -325,7 +325,7 @@ def run_ours(args):
                                 f"({n_rot * spec_bytes / 1e6:.0f} MB) so no flush is needed",
                           "parallelism": f"{world} x independent spectra (no collective)"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
-        if not args.no_cpu_baseline and world >= 1:
+        if not args.no_cpu_baseline and world == 1:  # rank 0 at N = 1 only
             cb, _, _ = cpu_baseline(wl, rows=args.cpu_rows)
             cb.pop("seconds", None)
             out["cpu_baseline"] = cb
