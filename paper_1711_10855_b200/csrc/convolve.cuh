@@ -186,15 +186,24 @@ template <class C> __device__ __forceinline__ void forward_to_inv_layout(float2 
     constexpr int RL = C::R(C::P - 1), BL = C::E / RL;
     fwd_from<C, 0>(v, buf0, buf1, tw, t);
     __syncthreads();
+    // element of natural frequency f sits at f + f/16: both index maps step through f in strides of 16
+    // within a half-warp, which the extra element per 16 spreads over the banks
+    static_assert(I::BUF_ELEMS >= C::L + C::L / 16, "re-layout buffer");
 #pragma unroll
     for (int b = 0; b < BL; ++b)
 #pragma unroll
-        for (int d = 0; d < RL; ++d) buf0[nat_freq<C>(t, b, d)] = v[b * RL + d];
+        for (int d = 0; d < RL; ++d) {
+            const int f = nat_freq<C>(t, b, d);
+            buf0[f + (f >> 4)] = v[b * RL + d];
+        }
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < I::NB; ++i)
 #pragma unroll
-        for (int k = 0; k < I::Ra; ++k) v[i * I::Ra + k] = buf0[inv_freq<C>(t, i, k)];
+        for (int k = 0; k < I::Ra; ++k) {
+            const int f = inv_freq<C>(t, i, k);
+            v[i * I::Ra + k] = buf0[f + (f >> 4)];
+        }
 }
 
 struct ConvParams {
