@@ -223,11 +223,11 @@ def test_repeated_launches_are_bitwise_identical(torch, binding, L, m):
     plan = binding.Plan(n_f, 40, 2, m, L, n_batch=3)
     plan.set_templates(H)
     d_spec = torch.from_numpy(spec).cuda()
-    outs = [torch.full((3, 41, n_f), float("nan"), dtype=torch.float32, device="cuda") for _ in range(6)]
-    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [torch.full((3, 41, n_f), float("nan"), dtype=torch.float32, device="cuda") for _ in range(12)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()]
     torch.cuda.synchronize()
-    for i, o in enumerate(outs):
-        plan.convolve(d_spec, o, stream=streams[i % 2])
+    for i, o in enumerate(outs):      # three streams: CTAs of different launches share SMs, large warp skews
+        plan.convolve(d_spec, o, stream=streams[i % 3])
     torch.cuda.synchronize()
     for o in outs[1:]:
         assert torch.equal(outs[0], o)
