@@ -110,6 +110,7 @@ int fdas_plan_nz(const fdas_plan *plan);            /* n_z */
 int fdas_plan_step(const fdas_plan *plan);          /* S = outputs kept per segment */
 int64_t fdas_plan_nseg(const fdas_plan *plan);      /* segments per spectrum */
 int fdas_plan_batch(const fdas_plan *plan);         /* n_batch */
+int fdas_plan_grid(const fdas_plan *plan);          /* CTAs of the persistent hot kernel: resident CTAs per SM x SMs */
 
 /* Number of kernel launches the last fdas_convolve on this plan made (bench.py "gpu_launches"). */
 int fdas_plan_last_launch_count(const fdas_plan *plan);

@@ -27,6 +27,7 @@ SYMBOLS = {
     "fdas_plan_step": (_int, [_vp]),
     "fdas_plan_nseg": (_i64, [_vp]),
     "fdas_plan_batch": (_int, [_vp]),
+    "fdas_plan_grid": (_int, [_vp]),
     "fdas_plan_last_launch_count": (_int, [_vp]),
     "fdas_plan_last_cuda_error": (_int, [_vp]),
     "fdas_status_string": (ctypes.c_char_p, [_int]),
@@ -113,6 +114,8 @@ class Plan:
     def n_seg(self): return lib().fdas_plan_nseg(self._h)
     @property
     def n_batch(self): return lib().fdas_plan_batch(self._h)
+    @property
+    def grid(self): return lib().fdas_plan_grid(self._h)
     @property
     def last_launch_count(self): return lib().fdas_plan_last_launch_count(self._h)
     @property

@@ -15,6 +15,8 @@
 // The z loop is software pipelined: stage A of template z+1 runs before the barrier of template z.
 // Measured cost model, ablations and the experiments that did not help: profiles/r1_c3_v4.md.
 #pragma once
+#include <type_traits>
+
 #include "fft_device.cuh"
 #include "sm100_ptx.cuh"
 
@@ -179,12 +181,13 @@ template <class C> struct TwTmem {
 
 // forward transform of v (natural order, v[d] = x[d*NT + t]) into layout P-1 of the inverse:
 // the decimation-in-frequency passes of fft_device.cuh followed by one re-layout through buf0.
-template <class C> __device__ __forceinline__ void forward_to_inv_layout(float2 *v, float2 *buf0, float2 *buf1,
-                                                                         const float2 *__restrict__ tw, int t)
+// REGS_DONE: the caller has already run fwd_pass_regs<C, 0> on v.
+template <class C, bool REGS_DONE = false>
+__device__ __forceinline__ void forward_to_inv_layout(float2 *v, float2 *buf0, float2 *buf1, const float2 *__restrict__ tw, int t)
 {
     using I = InvCfg<C>;
     constexpr int RL = C::R(C::P - 1), BL = C::E / RL;
-    fwd_from<C, 0>(v, buf0, buf1, tw, t);
+    fwd_from<C, 0, REGS_DONE>(v, buf0, buf1, tw, t);
     __syncthreads();
     // element of natural frequency f sits at f + f/16: both index maps step through f in strides of 16
     // within a half-warp, which the extra element per 16 spreads over the banks
@@ -211,11 +214,14 @@ struct ConvParams {
     float *__restrict__ power;           // [n_batch][n_z][n_f]
     const float4 *__restrict__ gperm;    // [n_z][E/2][NT] : template spectra in register order
     const float2 *__restrict__ tw;       // [L] : w_L^j
+    unsigned int *__restrict__ work;     // [2] : next work item, CTAs finished (both 0 between launches)
     int64_t n_f;
     int64_t n_seg;
+    int64_t n_work;                      // n_batch * n_seg
     int n_z;
     int m;
     int S;
+    int bulk_ok;                         // spectrum base is 16-byte aligned: interior segments may be bulk-copied
 };
 
 template <class C> constexpr size_t conv_smem_bytes()
@@ -223,6 +229,10 @@ template <class C> constexpr size_t conv_smem_bytes()
     return 2 * sizeof(float2) * (size_t)InvCfg<C>::BUF_ELEMS + sizeof(float2) * (size_t)C::L;
 }
 
+// Persistent kernel: the grid is one wave of resident CTAs (fdas.cu sizes it from the occupancy and
+// the tensor-memory budget); every CTA sets up its tensor-memory tables once and then takes
+// (batch item, segment) work items from a global counter until none is left.  Dynamic rather than
+// strided assignment because the CTAs sharing an SM do not run at the same speed (profiles/r1_c3_v5.md).
 template <int L>
 __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convolve_kernel(const ConvParams p)
 {
@@ -231,48 +241,30 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     using TC = TmemCfg<C>;
     constexpr int E = C::E, NT = C::NT;
     constexpr uint32_t G_BYTES = (uint32_t)L * 8u;
+    constexpr int D0_FAST = E / 8;       // first kept register when m = L/8 (every BASELINE.json config)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *buf0 = reinterpret_cast<float2 *>(smem_raw);
     float2 *buf1 = buf0 + I::BUF_ELEMS;
-    float4 *gs = reinterpret_cast<float4 *>(buf1 + I::BUF_ELEMS); // [E/2][NT]
+    float4 *gs = reinterpret_cast<float4 *>(buf1 + I::BUF_ELEMS); // [E/2][NT]: template stage / segment stage
     __shared__ __align__(8) uint64_t g_bar;
     __shared__ uint32_t tmem_slot;
+    __shared__ uint32_t s_work[2];
 
     const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
-    const int64_t seg = blockIdx.x % p.n_seg;
-    const int64_t bi = blockIdx.x / p.n_seg;
 
     if (t == 0) {
         ptx::mbar_init(&g_bar, 1);
         ptx::mbar_fence_init();
+        s_work[0] = atomicAdd(p.work, 1u);
     }
     if (warp == 0) ptx::tmem_alloc<TC::NCOLS>(&tmem_slot);
     ptx::tmem_fence_before_sync();
     __syncthreads();
     ptx::tmem_fence_after_sync();
-    if (t == 0) { // template spectrum of z = 0 (a3), in flight during the forward transform
-        ptx::mbar_expect_tx(&g_bar, G_BYTES);
-        ptx::bulk_g2s(gs, p.gperm, G_BYTES, &g_bar);
-    }
     const uint32_t tm_addr = tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(TC::SLOT_COLS * (warp >> 2));
 
-    // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
-    float2 v[E];
-    {
-        const float2 *__restrict__ A = p.spectrum + bi * p.n_f;
-        const int64_t base = seg * p.S - p.m / 2;
-#pragma unroll
-        for (int d = 0; d < E; ++d) {
-            const int64_t k = base + d * NT + t;
-            v[d] = (k >= 0 && k < p.n_f) ? __ldg(A + k) : make_float2(0.f, 0.f);
-        }
-    }
-    // a2: forward FFT, once per segment (eq.(3)); the result is parked in tensor memory
-    forward_to_inv_layout<C>(v, buf0, buf1, p.tw, t);
-    ptx::tmem_st16(tm_addr + TC::X_OFF, v);
-    if constexpr (E > 8) ptx::tmem_st16(tm_addr + TC::X_OFF + 16, v + 8);
-
-    // inverse multipliers (independent of z): pass 0 in registers, the others in tensor memory
+    // inverse multipliers (independent of z and of the segment): once per CTA.  Pass 0 in
+    // registers for the 64-thread plans, everything else in tensor memory.
     float2 tw0[TC::TW0_PARKED ? 1 : C::R(0)];
     {
         if constexpr (TC::TW0_PARKED) {
@@ -298,74 +290,160 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
             ptx::tmem_st16(tm_addr + TC::TWM_OFF, w);
         }
     }
-    ptx::tmem_wait_st();
-
     const InvAddr<C> A = inv_addr<C>(t);
     TwTmem<C> tws{tm_addr};
+    uint32_t gphase = 0; // parity of the next completion of g_bar
+    const bool fast_m = (p.m * 8 == L);
 
-    const int64_t col0 = seg * p.S - p.m + t;                 // column of y[t]
-    float *__restrict__ prow = p.power + bi * p.n_z * p.n_f;  // row 0 of this batch item
-    const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
-    const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
-    const int d0 = p.m / NT;
-
-    // a3 + first inverse pass of template z ("convolution in the Fourier domain"; "for every
-    // matched filter"): v = X * G_z in layout P-1, butterflies of pass P-1
-    auto stage_a = [&](int z) {
-        float2 X[E];
-        ptx::tmem_ld16(tm_addr + TC::X_OFF, X);
-        if constexpr (E > 8) ptx::tmem_ld16(tm_addr + TC::X_OFF + 16, X + 8);
-        ptx::mbar_wait(&g_bar, (uint32_t)(z & 1));
-        ptx::tmem_wait_ld8(X);
-        if constexpr (E > 8) ptx::tmem_wait_ld8(X + 8);
-#pragma unroll
-        for (int q = 0; q < E / 2; ++q) {
-            const float4 g = gs[q * NT + t];
-            v[2 * q] = cmul(X[2 * q], make_float2(g.x, g.y));
-            v[2 * q + 1] = cmul(X[2 * q + 1], make_float2(g.z, g.w));
-        }
-        inv_stage_a<C>(v);
+    // a1 through the bulk-copy engine: segment `w` can be copied as one 16-byte aligned block of L
+    // complex64 if it lies inside [0, n_f); the first and last segment(s) need the zero padding of
+    // reading 6 and are loaded with guarded loads instead.
+    auto seg_base = [&](uint32_t w) { return (int64_t)(w % p.n_seg) * p.S - p.m / 2; };
+    auto seg_bulk = [&](uint32_t w) {
+        const int64_t base = seg_base(w);
+        return p.bulk_ok && base >= 0 && base + L <= p.n_f && (((w / p.n_seg) * p.n_f + base) & 1) == 0;
     };
-    auto fetch_g = [&](int z) { // elected thread: bulk copy of G_z into the stage (every thread is past its reads)
-        if (t == 0 && z < p.n_z) {
-            ptx::mbar_expect_tx(&g_bar, G_BYTES);
-            ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)z * G_BYTES, G_BYTES, &g_bar);
-        }
+    auto fetch_segment = [&](uint32_t w) { // elected thread
+        const float2 *src = p.spectrum + (int64_t)(w / p.n_seg) * p.n_f + seg_base(w);
+        ptx::mbar_expect_tx(&g_bar, G_BYTES);
+        ptx::bulk_g2s(gs, src, G_BYTES, &g_bar);
     };
-    stage_a(0);
-    __syncthreads(); // also: the forward transform's last reads of buf0 are done before the z loop writes it
-    fetch_g(1);
 
-    // The z loop is software pipelined: stage A of template z+1 (tensor-memory and shared-memory
-    // reads, 1/3 of the arithmetic) sits between the exchange write of template z and its barrier, so
-    // a warp that reaches the barrier early has independent work instead of idling.
-    for (int z = 0; z < p.n_z; ++z) {
-        float2 *bufa = (C::P == 3 && (z & 1)) ? buf1 : buf0;
-        inv_stage_b<C>(v, bufa, A, tws, lane);
-        if (z + 1 < p.n_z) stage_a(z + 1);
-        __syncthreads();
-        fetch_g(z + 2);
-        float2 u[E];
-        inv_stage_c<C>(u, bufa, buf1, A, tw0, tws);
-        // a5 + a6: trim, power, coalesced store
-        float *__restrict__ out = prow + (int64_t)z * p.n_f + col0;
-        if (fast) {
+    uint32_t w = s_work[0];
+    int slot = 0;
+    if (t == 0 && w < p.n_work && seg_bulk(w)) fetch_segment(w);
+
+    while (w < p.n_work) {
+        const int64_t seg = w % p.n_seg;
+        const int64_t bi = w / p.n_seg;
+        uint32_t w_next = 0;
+        if (t == 0) w_next = atomicAdd(p.work, 1u); // consumed after the first barrier below
+
+        // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
+        float2 v[E];
+        if (seg_bulk(w)) {
+            ptx::mbar_wait(&g_bar, gphase);
+            gphase ^= 1;
+            const float2 *xs = reinterpret_cast<const float2 *>(gs);
 #pragma unroll
-            for (int d = 0; d < E; ++d) {
-                if (d >= 4 || d >= d0) __stcs(out + d * NT, u[d].x * u[d].x + u[d].y * u[d].y);
-            }
+            for (int d = 0; d < E; ++d) v[d] = xs[d * NT + t];
         } else {
+            const float2 *__restrict__ Ab = p.spectrum + bi * p.n_f;
+            const int64_t base = seg * p.S - p.m / 2;
 #pragma unroll
             for (int d = 0; d < E; ++d) {
-                const int pidx = d * NT + t;
-                const int64_t col = col0 + d * NT;
-                if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = u[d].x * u[d].x + u[d].y * u[d].y;
+                const int64_t k = base + d * NT + t;
+                v[d] = (k >= 0 && k < p.n_f) ? __ldg(Ab + k) : make_float2(0.f, 0.f);
             }
         }
+        // a2: forward FFT, once per segment (eq.(3)); the result is parked in tensor memory.  The register
+        // part of its first pass comes before the barrier that releases the stage to the bulk-copy engine:
+        // the engine does not queue behind this thread's loads, so they must have returned (been used)
+        // before the thread arrives.
+        fwd_pass_regs<C, 0>(v, p.tw, t);
+        __syncthreads(); // the stage is read; the previous item's last exchange reads are done
+        if (t == 0) {    // template spectrum of z = 0 (a3), in flight during the forward transform
+            ptx::mbar_expect_tx(&g_bar, G_BYTES);
+            ptx::bulk_g2s(gs, p.gperm, G_BYTES, &g_bar);
+        }
+        forward_to_inv_layout<C, true>(v, buf0, buf1, p.tw, t);
+        ptx::tmem_st16(tm_addr + TC::X_OFF, v);
+        if constexpr (E > 8) ptx::tmem_st16(tm_addr + TC::X_OFF + 16, v + 8);
+        ptx::tmem_wait_st();
+
+        const int64_t col0 = seg * p.S - p.m + t;                             // column of y[t]
+        float *__restrict__ out = p.power + bi * p.n_z * p.n_f + col0;        // row 0 of this batch item
+        const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
+        const bool fast8 = interior && fast_m;
+        const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
+        const int d0 = p.m / NT;
+
+        // a3 + first inverse pass of template z ("convolution in the Fourier domain"; "for every
+        // matched filter"): v = X * G_z in layout P-1, butterflies of pass P-1
+        auto stage_a = [&]() {
+            float2 X[E];
+            ptx::tmem_ld16(tm_addr + TC::X_OFF, X);
+            if constexpr (E > 8) ptx::tmem_ld16(tm_addr + TC::X_OFF + 16, X + 8);
+            ptx::mbar_wait(&g_bar, gphase);
+            gphase ^= 1;
+            ptx::tmem_wait_ld8(X);
+            if constexpr (E > 8) ptx::tmem_wait_ld8(X + 8);
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) {
+                const float4 g = gs[q * NT + t];
+                v[2 * q] = cmul(X[2 * q], make_float2(g.x, g.y));
+                v[2 * q + 1] = cmul(X[2 * q + 1], make_float2(g.z, g.w));
+            }
+            inv_stage_a<C>(v);
+        };
+        // elected thread, every thread being past its reads of the stage: slot k < n_z is the template
+        // spectrum G_k, slot n_z the next work item's segment
+        auto fetch_slot = [&](int k) {
+            if (t == 0) {
+                if (k < p.n_z) {
+                    ptx::mbar_expect_tx(&g_bar, G_BYTES);
+                    ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)k * G_BYTES, G_BYTES, &g_bar);
+                } else if (k == p.n_z && w_next < p.n_work && seg_bulk(w_next)) {
+                    fetch_segment(w_next);
+                }
+            }
+        };
+        stage_a();
+        __syncthreads(); // also: the forward transform's last reads of buf0 are done before the z loop writes it
+        if (t == 0) s_work[slot ^ 1] = w_next;
+        fetch_slot(1);
+
+        // The z loop is software pipelined: stage A of template z+1 (tensor-memory and shared-memory
+        // reads, 1/3 of the arithmetic) sits between the exchange write of template z and its barrier, so
+        // a warp that reaches the barrier early has independent work instead of idling.  The loop exists
+        // once per store mode (a5 + a6 below) so that the mode costs nothing inside it.
+        auto z_loop = [&](auto mode_tag) {
+            constexpr int MODE = decltype(mode_tag)::value;
+            for (int z = 0; z < p.n_z; ++z) {
+                float2 *bufa = (C::P == 3 && (z & 1)) ? buf1 : buf0;
+                inv_stage_b<C>(v, bufa, A, tws, lane);
+                if (z + 1 < p.n_z) stage_a();
+                __syncthreads();
+                fetch_slot(z + 2);
+                float2 u[E];
+                inv_stage_c<C>(u, bufa, buf1, A, tw0, tws);
+                // a5 + a6: trim, power, coalesced store
+                if constexpr (MODE == 0) {        // interior segment, m = L/8: registers D0_FAST.. are kept
+#pragma unroll
+                    for (int d = D0_FAST; d < E; ++d) __stcs(out + d * NT, u[d].x * u[d].x + u[d].y * u[d].y);
+                } else if constexpr (MODE == 1) { // interior segment, m a small multiple of the thread count
+#pragma unroll
+                    for (int d = 0; d < E; ++d) {
+                        if (d >= 4 || d >= d0) __stcs(out + d * NT, u[d].x * u[d].x + u[d].y * u[d].y);
+                    }
+                } else {                          // anything else: per-element bounds
+#pragma unroll
+                    for (int d = 0; d < E; ++d) {
+                        const int pidx = d * NT + t;
+                        const int64_t col = col0 + d * NT;
+                        if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = u[d].x * u[d].x + u[d].y * u[d].y;
+                    }
+                }
+                out += p.n_f;
+            }
+        };
+        if (fast8) z_loop(std::integral_constant<int, 0>{});
+        else if (fast) z_loop(std::integral_constant<int, 1>{});
+        else z_loop(std::integral_constant<int, 2>{});
+        slot ^= 1;
+        w = s_work[slot];
     }
     ptx::tmem_fence_before_sync();
     __syncthreads();
     if (warp == 0) ptx::tmem_free<TC::NCOLS>(tmem_slot);
+    if (t == 0) { // the last CTA out re-arms the counters for the next launch
+        __threadfence();
+        if (atomicAdd(p.work + 1, 1u) == gridDim.x - 1) {
+            p.work[0] = 0;
+            p.work[1] = 0;
+            __threadfence();
+        }
+    }
 }
 
 } // namespace fdas

@@ -121,6 +121,10 @@ struct fdas_plan {
     bool has_templates;
     int last_cuda_error;
     int last_launches;
+    int device;               // CUDA device the plan lives on (every call checks it)
+    int grid_max;             // resident CTAs of the hot kernel on this device (registers, smem, tensor memory)
+    unsigned int *d_work;     // [WORK_SLOTS][2] work counters of the persistent kernel, zero between launches
+    unsigned int work_seq;    // launches so far: selects the counter pair
     // buffers of fdas_convolve_host
     void *d_host_spec;
     float *d_host_power;
@@ -157,21 +161,56 @@ cudaError_t upload_twiddles(int L, float2 **d_tw)
 
 template <int L> size_t smem_bytes() { return 2 * sizeof(float2) * (size_t)InvCfg<Cfg<L>>::BUF_ELEMS; }
 
-template <int L> cudaError_t launch_convolve(const ConvParams &cp, int n_batch, cudaStream_t st)
+// Counter pairs of the persistent kernel.  Launches take them round robin, so launches of one plan
+// that run concurrently (several streams) use different pairs; a pair is re-armed by its own launch.
+constexpr unsigned WORK_SLOTS = 1024;
+
+template <int L> cudaError_t launch_convolve(const ConvParams &cp, int grid_max, cudaStream_t st)
 {
     auto kern = fdas_convolve_kernel<L>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
-    const int64_t blocks = cp.n_seg * n_batch;
-    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    kern<<<(unsigned)blocks, Cfg<L>::NT, smem, st>>>(cp);
+    if (cp.n_work > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    const unsigned grid = (unsigned)(cp.n_work < grid_max ? cp.n_work : grid_max);
+    kern<<<grid, Cfg<L>::NT, smem, st>>>(cp);
     return cudaGetLastError();
 }
 
-// opt the hot kernel of this segment length in to its dynamic shared memory (once per plan, at creation)
-template <int L> cudaError_t prepare_convolve()
+// Once per plan, at creation: opt the hot kernel of this segment length in to its dynamic shared
+// memory and size the persistent grid = resident CTAs per SM x SMs.  Resident CTAs are counted here
+// from the kernel's registers and shared memory, the SM's thread / block limits and the tensor memory
+// (512 columns per SM); the occupancy API reports one CTA per SM for a kernel that allocates tensor memory.
+template <int L> cudaError_t prepare_convolve(int device, int *grid_max)
 {
-    return cudaFuncSetAttribute(fdas_convolve_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)conv_smem_bytes<Cfg<L>>());
+    auto kern = fdas_convolve_kernel<L>;
+    constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
+    constexpr int NT = Cfg<L>::NT;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    int n_sm = 0, regs_sm = 0, smem_sm = 0, smem_rsv = 0, thr_sm = 0, blk_sm = 0;
+    const cudaDeviceAttr attr[6] = {cudaDevAttrMultiProcessorCount, cudaDevAttrMaxRegistersPerMultiprocessor,
+                                    cudaDevAttrMaxSharedMemoryPerMultiprocessor, cudaDevAttrReservedSharedMemoryPerBlock,
+                                    cudaDevAttrMaxThreadsPerMultiProcessor, cudaDevAttrMaxBlocksPerMultiprocessor};
+    int *dst[6] = {&n_sm, &regs_sm, &smem_sm, &smem_rsv, &thr_sm, &blk_sm};
+    for (int i = 0; i < 6; ++i) {
+        e = cudaDeviceGetAttribute(dst[i], attr[i], device);
+        if (e != cudaSuccess) return e;
+    }
+    const int regs_cta = ((fa.numRegs + 7) / 8 * 8) * NT;       // registers are allocated per warp in units of 256
+    const int smem_cta = (int)smem + (int)fa.sharedSizeBytes + smem_rsv;
+    int per_sm = regs_sm / regs_cta;
+    if (per_sm > smem_sm / smem_cta) per_sm = smem_sm / smem_cta;
+    if (per_sm > thr_sm / NT) per_sm = thr_sm / NT;
+    if (per_sm > blk_sm) per_sm = blk_sm;
+    if (per_sm > 512 / TmemCfg<Cfg<L>>::NCOLS) per_sm = 512 / TmemCfg<Cfg<L>>::NCOLS;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    *grid_max = per_sm * n_sm;
+    if (const char *g = getenv("FDAS_EXP_GRID")) *grid_max = atoi(g);
+    return cudaSuccess;
 }
 
 template <int L> cudaError_t launch_template_fft(const float2 *d_h, int m, int n_z, const float2 *d_tw, float4 *d_g)
@@ -263,17 +302,21 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
     p->S = segment_len - template_width;
     p->n_seg = (n_f + p->S - 1) / p->S;
     p->n_batch = 1;
-    cudaError_t e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
     if (e == cudaSuccess) e = upload_twiddles(p->L, &p->d_tw);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_work, sizeof(unsigned int) * 2 * WORK_SLOTS);
+    if (e == cudaSuccess) e = cudaMemset(p->d_work, 0, sizeof(unsigned int) * 2 * WORK_SLOTS);
     if (e == cudaSuccess) {
         const int L = p->L;
-        FDAS_DISPATCH_L(L, e = prepare_convolve<LL>());
+        FDAS_DISPATCH_L(L, e = prepare_convolve<LL>(p->device, &p->grid_max));
     }
     if (e != cudaSuccess) {
         fdas_status s = (e == cudaErrorMemoryAllocation) ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
         (void)cudaGetLastError();
         if (p->d_gperm) cudaFree(p->d_gperm);
         if (p->d_tw) cudaFree(p->d_tw);
+        if (p->d_work) cudaFree(p->d_work);
         free(p);
         return s;
     }
@@ -317,15 +360,18 @@ fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, 
     cp.power = d_power;
     cp.gperm = p->d_gperm;
     cp.tw = p->d_tw;
+    cp.work = p->d_work + 2 * (p->work_seq++ % WORK_SLOTS);
     cp.n_f = p->n_f;
     cp.n_seg = p->n_seg;
+    cp.n_work = p->n_seg * (int64_t)p->n_batch;
     cp.n_z = p->n_z;
     cp.m = p->m;
     cp.S = p->S;
+    cp.bulk_ok = ((uintptr_t)d_spectrum & 15u) == 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
-    FDAS_DISPATCH_L(L, (e = launch_convolve<LL>(cp, p->n_batch, st)));
+    FDAS_DISPATCH_L(L, (e = launch_convolve<LL>(cp, p->grid_max, st)));
     p->last_launches = 1;
     if (e != cudaSuccess) return cuda_fail(p, e);
     return FDAS_OK;
@@ -368,6 +414,7 @@ fdas_status fdas_plan_destroy(fdas_plan *p)
     if (!p) return FDAS_OK;
     if (p->d_gperm) cudaFree(p->d_gperm);
     if (p->d_tw) cudaFree(p->d_tw);
+    if (p->d_work) cudaFree(p->d_work);
     if (p->d_host_spec) cudaFree(p->d_host_spec);
     if (p->d_host_power) cudaFree(p->d_host_power);
     (void)cudaGetLastError();
@@ -379,6 +426,7 @@ int fdas_plan_nz(const fdas_plan *p) { return p ? p->n_z : 0; }
 int fdas_plan_step(const fdas_plan *p) { return p ? p->S : 0; }
 int64_t fdas_plan_nseg(const fdas_plan *p) { return p ? p->n_seg : 0; }
 int fdas_plan_batch(const fdas_plan *p) { return p ? p->n_batch : 0; }
+int fdas_plan_grid(const fdas_plan *p) { return p ? p->grid_max : 0; }
 int fdas_plan_last_launch_count(const fdas_plan *p) { return p ? p->last_launches : 0; }
 int fdas_plan_last_cuda_error(const fdas_plan *p) { return p ? p->last_cuda_error : -1; }
 

@@ -147,11 +147,8 @@ template <class C, int I, bool INV> __device__ __forceinline__ void butterflies(
     for (int b = 0; b < B; ++b) Dft<R, INV>::run(v + b * R);
 }
 
-// Forward passes I..P-1 (recursive over compile-time I).  v enters in layout I (already loaded).
-// bufs: two exchange buffers used alternately.  Ends in layout P-1.  Barriers: one before each
-// write (WAR on the buffer pair is covered by the caller for the first write) and one after.
-template <class C, int I> __device__ __forceinline__ void fwd_from(float2 *v, float2 *buf0, float2 *buf1,
-                                                                   const float2 *__restrict__ tw, int t)
+// Register part of forward pass I: butterflies of digit I, then the twiddles w_{R_I Lo_I}^{k_I low}.
+template <class C, int I> __device__ __forceinline__ void fwd_pass_regs(float2 *v, const float2 *__restrict__ tw, int t)
 {
     butterflies<C, I, false>(v);
     if constexpr (I < C::P - 1) {
@@ -163,6 +160,18 @@ template <class C, int I> __device__ __forceinline__ void fwd_from(float2 *v, fl
 #pragma unroll
             for (int b = 0; b < B; ++b) v[b * R + d] = cmul(v[b * R + d], w);
         }
+    }
+}
+
+// Forward passes I..P-1 (recursive over compile-time I).  v enters in layout I (already loaded);
+// REGS_DONE: the caller has already run fwd_pass_regs<C, I>.  bufs: two exchange buffers used
+// alternately.  Ends in layout P-1.  Barriers: one before each write (WAR on the buffer pair is
+// covered by the caller for the first write) and one after.
+template <class C, int I, bool REGS_DONE = false>
+__device__ __forceinline__ void fwd_from(float2 *v, float2 *buf0, float2 *buf1, const float2 *__restrict__ tw, int t)
+{
+    if constexpr (!REGS_DONE) fwd_pass_regs<C, I>(v, tw, t);
+    if constexpr (I < C::P - 1) {
         float2 *buf = (I & 1) ? buf1 : buf0;
         sm_write<C, I>(buf, lay_base<C, I>(t), v);
         __syncthreads();
