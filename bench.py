@@ -32,14 +32,26 @@ UNIT = "points/s"
 FP32_LANES_PER_SM = 128  # B200: 4 SMSPs x 32 FP32 lanes, 2 flops per FMA
 N_SM = 148
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the hot kernel, from the committed
-# `ncu --set full` capture named here (None until a capture exists for that workload).
-NCU_TRAFFIC = {
-    "C3": (3313898000 + 40858112, "profiles/r1_c3_v5.md"),
-}
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
 
 
-def parse_args():
+def ncu_traffic(workload_name, kernel_version):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the hot kernel from the committed
+    `ncu --set full` capture of THIS kernel version (profiles/traffic.json, written by hand from the
+    capture named there).  None when the library's kernel version has no capture: a stale figure is
+    worse than none."""
+    try:
+        with open(TRAFFIC_JSON) as f:
+            table = json.load(f)
+    except (OSError, ValueError):
+        return None, None
+    e = table.get(kernel_version, {}).get(workload_name)
+    if not e:
+        return None, None
+    return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"]), e.get("source")
+
+
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
@@ -50,7 +62,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the plane the oracle is timed on (0 = auto)")
-    return ap.parse_args()
+    ap.add_argument("--dry-run", action="store_true",
+                    help="no GPU: exercise the launcher, the gloo rendezvous and the cross-rank timing reduction only")
+    return ap.parse_args(argv)
 
 
 def peaks():
@@ -298,7 +312,7 @@ def run_ours(args):
         t_alu = flops_alg / (fp32_peak * 1e12)
         t_hbm = bytes_alg / (pk["hbm_gbs"] * 1e9)
         alu_binds = t_alu >= t_hbm
-        traffic = NCU_TRAFFIC.get(wl.name.split("[")[0], (None, None))
+        traffic = ncu_traffic(wl.name, binding.version())
         roofline = {
             "bound": "alu" if alu_binds else "hbm",
             "achieved": ach_tf if alu_binds else ach_gb,
@@ -337,10 +351,52 @@ def run_ours(args):
     return 0
 
 
+def run_dry(args):
+    """--dry-run: everything of the N-rank path that needs no GPU (gloo): rendezvous, per-rank seeded
+    workload shape, MAX-over-ranks of a per-rank time, whole-job value.  Prints the JSON line with
+    "dry_run": true; its `value` is meaningless."""
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    from paper_1711_10855_b200 import workload
+    shape = workload.config_shape(args.config, pair=args.pair if args.config == 4 else 0)
+    points = shape["n_batch"] * shape["n_z"] * shape["n_f"]
+    t_ms = max_over_ranks(1.0 + rank, world)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": whole_job_value(points, world, args.steps, t_ms * args.steps),
+                          "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "dry_run": True,
+                          "ms_per_step": t_ms, "higher_is_better": True, "scaling": "weak", "data": "synthetic",
+                          "config": {"workload": shape["name"], "parallelism": f"{world} x independent spectra (no collective)"}}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, one per GPU, exactly as
+    the driver does (torch.distributed.run, one node, rendezvous on 127.0.0.1)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "VERSION")  # one line per job: the NCCL version, visible in stderr
+    return subprocess.call(cmd, env=env)
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return relaunch_under_torchrun(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.dry_run:
+        return run_dry(args)
     return run_ours(args)
 
 

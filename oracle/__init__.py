@@ -40,6 +40,8 @@ def lib():
         L.fdas_oracle_direct.restype = ctypes.c_int
         L.fdas_oracle_ols.argtypes = [dp, i64, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                       ctypes.c_int, ctypes.c_int, dp]
+        L.fdas_oracle_blockmax.argtypes = [dp, ctypes.c_int, i64, i64, ctypes.c_int, dp, ctypes.POINTER(ctypes.c_int64)]
+        L.fdas_oracle_blockmax.restype = ctypes.c_int
         L.fdas_oracle_ols.restype = ctypes.c_int
         _LIB = L
     return _LIB
@@ -140,3 +142,23 @@ def ols(spectrum, templates_, seg_len, step=None, rows=None):
     if rc != 0:
         raise ValueError("oracle ols: bad arguments")
     return p
+
+
+def blockmax(power, blk, float32_decision=True):
+    """Detection step over a power plane [rows][cols] (reading 17): per row and block of `blk`
+    columns the maximum and the lowest in-block offset attaining it.  Returns (float64 [rows][n_blk],
+    int64 [rows][n_blk]).  float32_decision: compare float32-rounded powers (the CUDA path's precision)."""
+    p = np.ascontiguousarray(power, dtype=np.float64)
+    if p.ndim != 2:
+        raise ValueError("power must be [rows][cols]")
+    n_rows, n_cols = p.shape
+    if int(blk) < 1 or n_cols < 1:
+        raise ValueError("oracle blockmax: bad arguments")
+    n_blk = (n_cols + int(blk) - 1) // int(blk)
+    mx = np.empty((n_rows, n_blk), dtype=np.float64)
+    ar = np.empty((n_rows, n_blk), dtype=np.int64)
+    rc = lib().fdas_oracle_blockmax(_dp(p), n_rows, n_cols, int(blk), int(bool(float32_decision)), _dp(mx),
+                                    ar.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)))
+    if rc != 0:
+        raise ValueError("oracle blockmax: bad arguments")
+    return mx, ar

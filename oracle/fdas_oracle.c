@@ -19,11 +19,16 @@
  *                                         and its power |A'|^2 (the authority for parity)
  *   fdas_oracle_ols        P:31           the same plane by overlap-and-save in double, with
  *                                         fdas_oracle_fft (checked against fdas_oracle_direct)
+ *   fdas_oracle_blockmax   P:21, P:50     the detection step that consumes the plane ("FDAS code";
+ *                                         the paper leaves it to Dimoudi 2017, reading 17):
+ *                                         per row and block of columns, the maximum power and the
+ *                                         lowest column that attains it
  *
  * Pins (tests/test_oracle_*.py): brute-force DFT vs FFT; Parseval; scipy.special.fresnel; an
  * independent quadrature of the defining integral; the DFT of a sampled chirp; z=0 -> delta;
  * numpy.convolve; impulse / constant inputs with closed forms; an injected signal peaking in
- * its row; linearity; OLS == direct.  Nothing in this file is "parity unpinned".
+ * its row; linearity; OLS == direct; block maxima against a Python loop, numpy and the C1 peak.
+ * Nothing in this file is "parity unpinned".
  *
  * Complex arrays are interleaved (re, im) doubles.  No function here reorders, blocks or fuses
  * beyond what the cited definition states, except that fdas_oracle_direct walks columns in
@@ -355,4 +360,34 @@ int fdas_oracle_ols(const double *spectrum, int64_t n_f, const double *templates
     }
     free(G);
     return fail ? -1 : 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Detection step over a power plane ("detect"; "FDAS code"; reading 17):
+ * for every row r and block b of `blk` consecutive columns, [b*blk, min((b+1)*blk, n_cols)),
+ *   max_out[r][b] = max_c P[r][c]        arg_out[r][b] = the smallest c - b*blk with P[r][c] = max
+ * n_blk = ceil(n_cols / blk).  in_float32 != 0: every power is rounded to IEEE float32 before
+ * it is compared (the precision in which the CUDA path takes the same decision); max_out then
+ * holds the rounded value.  Plain scan, left to right.
+ * ------------------------------------------------------------------------------------------ */
+int fdas_oracle_blockmax(const double *power, int n_rows, int64_t n_cols, int64_t blk, int in_float32,
+                         double *max_out, int64_t *arg_out)
+{
+    if (!power || !max_out || !arg_out || n_rows < 0 || n_cols < 1 || blk < 1) return -1;
+    int64_t n_blk = (n_cols + blk - 1) / blk;
+    for (int r = 0; r < n_rows; ++r) {
+        for (int64_t b = 0; b < n_blk; ++b) {
+            int64_t c0 = b * blk, c1 = c0 + blk < n_cols ? c0 + blk : n_cols;
+            double best = 0.0;
+            int64_t arg = -1;
+            for (int64_t c = c0; c < c1; ++c) {
+                double v = power[(size_t)r * (size_t)n_cols + (size_t)c];
+                if (in_float32) v = (double)(float)v;
+                if (arg < 0 || v > best) { best = v; arg = c - c0; }
+            }
+            max_out[(size_t)r * (size_t)n_blk + (size_t)b] = best;
+            arg_out[(size_t)r * (size_t)n_blk + (size_t)b] = arg;
+        }
+    }
+    return 0;
 }

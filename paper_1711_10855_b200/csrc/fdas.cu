@@ -135,6 +135,14 @@ namespace {
 
 bool supported_L(int L) { return L == 512 || L == 1024 || L == 2048 || L == 4096 || L == 8192; }
 
+// A plan lives on the device that was current at fdas_plan_create; every later call must be made
+// with that device current (its buffers, its opted-in kernel attributes).
+bool on_plan_device(const fdas_plan *p)
+{
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == p->device;
+}
+
 fdas_status cuda_fail(fdas_plan *p, cudaError_t e)
 {
     if (p) p->last_cuda_error = (int)e;
@@ -334,9 +342,13 @@ fdas_status fdas_plan_set_batch(fdas_plan *p, int n_batch)
 fdas_status fdas_set_templates(fdas_plan *p, const float *h_templates)
 {
     if (!p || !h_templates) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     const size_t bytes = sizeof(float2) * (size_t)p->n_z * (size_t)p->m;
     float2 *d_h = nullptr;
-    cudaError_t e = cudaMalloc((void **)&d_h, bytes);
+    // the bank is replaced in place: wait for every fdas_convolve still reading the old one (any stream)
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    e = cudaMalloc((void **)&d_h, bytes);
     if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
     e = cudaMemcpy(d_h, h_templates, bytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
@@ -354,6 +366,7 @@ fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, 
 {
     if (!p || !d_spectrum || !d_power) return FDAS_ERR_INVALID_ARG;
     if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_power & 3u)) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
     ConvParams cp;
     cp.spectrum = (const float2 *)d_spectrum;
@@ -466,6 +479,7 @@ int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b)
     return r;
 }
 
-const char *fdas_version(void) { return "libfdas sm_100a " __DATE__; }
+// The kernel generation is what profiles/traffic.json is keyed by: bump it with every change to the hot kernel.
+const char *fdas_version(void) { return "libfdas sm_100a k6"; }
 
 } // extern "C"

@@ -172,6 +172,12 @@ def make_config(c: int, pair: int = 0, n_batch: Optional[int] = None, n_f: Optio
     return Workload(name, nf, z_max, z_step, m, L, nb, spec, H, sigs)
 
 
+def config_shape(c: int, pair: int = 0) -> dict:
+    """Sizes of BASELINE.json config c without generating any data."""
+    wl = make_config(c, pair=pair, n_f=None, with_spectrum=False)
+    return {"name": wl.name, "n_f": wl.n_f, "n_z": wl.n_z, "m": wl.m, "seg_len": wl.seg_len, "n_batch": wl.n_batch}
+
+
 def noise_spectrum(n_f: int, seed: int, n_batch: int = 1) -> np.ndarray:
     """Plain N(0,1)+iN(0,1) complex64 [n_batch][n_f] (bench.py's bulk input; no signals)."""
     rng = np.random.Generator(np.random.PCG64(seed))

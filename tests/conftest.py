@@ -1,4 +1,5 @@
 import os
+import subprocess
 import sys
 
 import pytest
@@ -12,8 +13,12 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box via gpurun)")
     # a fresh checkout has no libfdas.so (built artefacts are git-ignored): build it once, in tree, with
     # nvcc for sm_100a (cross-compiles without a GPU).  The library itself never builds or falls back.
+    # On a host without nvcc the oracle tests still run; tests that load the library fail there.
     from paper_1711_10855_b200 import build as _build
-    _build.build()
+    try:
+        _build.build()
+    except (OSError, subprocess.CalledProcessError) as e:
+        print(f"conftest: could not build libfdas.so ({e}); only the oracle tests can run", file=sys.stderr)
 
 
 @pytest.fixture(scope="session")

@@ -57,3 +57,21 @@ def test_two_ranks_shard_by_spectrum_and_reduce_time_by_max():
         assert value == world * points * 4 / 5.0e-3
         assert abs(sums[0] - sums[1]) > 1.0                         # different seeded spectra per rank
     assert res[0][3] == res[1][3]
+
+
+def test_bench_launches_its_own_ranks():
+    """`python bench.py --gpus 2` with no launcher around it starts two ranks itself (torch.distributed.run on
+    127.0.0.1) -- here on the CPU-only --dry-run path (gloo), which shares the launcher, the rendezvous and the
+    MAX-over-ranks reduction with the GPU path."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run", "--steps", "4", "--config", "1"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout                      # rank 0 alone prints
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["dry_run"] is True
+    assert out["ms_per_step"] == 2.0                      # MAX over ranks of (1 + rank) ms
+    assert out["value"] == 2 * 33 * (1 << 16) * 4 / (2.0e-3 * 4)
