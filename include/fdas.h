@@ -76,7 +76,8 @@ fdas_status fdas_plan_set_batch(fdas_plan *plan, int n_batch);
  * The library conjugates the taps (eq.(2): conj(H)), zero-pads to L, scales by 1/L (the inverse
  * transform's factor, reading 9), transforms them with its own FFT kernel and stores the
  * spectra in the register order the convolution kernel reads.  Synchronous: returns after the
- * device work has finished.  May be called again to replace the bank.
+ * device work has finished.  May be called again to replace the bank: the call first waits for
+ * the whole device (cudaDeviceSynchronize), so work still reading the old bank finishes first.
  */
 fdas_status fdas_set_templates(fdas_plan *plan, const float *h_templates);
 
@@ -88,7 +89,11 @@ fdas_status fdas_set_templates(fdas_plan *plan, const float *h_templates);
  *                 alignment and n_f % 32 == 0 give fully coalesced line writes)
  *   cuda_stream   a cudaStream_t passed as void* (NULL = the legacy default stream)
  * Asynchronous: only launches; never synchronises, allocates or copies.  The buffers must stay
- * valid until the stream has run the work.  Output is bitwise reproducible (no atomics).
+ * valid until the stream has run the work.  Output is bitwise reproducible (the kernel hands out
+ * segments through an atomic counter, but which CTA computes a segment does not change its result).
+ * The plan may be used from several streams at once; at most 1024 launches of one plan may be
+ * in flight (enqueued and not finished) at any time: they take the plan's work counters round robin.
+ * Must be called with the plan's device current (the one current at fdas_plan_create).
  * Errors: INVALID_ARG (NULL / misaligned pointers), NO_TEMPLATES, CUDA (launch failure).
  */
 fdas_status fdas_convolve(fdas_plan *plan, const void *d_spectrum, float *d_power, void *cuda_stream);
@@ -96,11 +101,35 @@ fdas_status fdas_convolve(fdas_plan *plan, const void *d_spectrum, float *d_powe
 /*
  * Convenience for callers whose data live in HOST memory (bench.py's "e2e" leg): copies
  * h_spectrum to a plan-owned device buffer, runs fdas_convolve, copies the power plane back to
- * h_power, and synchronises the stream.  Buffers are allocated on first use and kept by the plan.
+ * h_power, and synchronises the stream.  Buffers are allocated on first use and kept by the plan:
+ * two *_host calls on one plan must not overlap (not from two host threads, not on two streams).
  *   h_spectrum    HOST (pinned memory gives asynchronous copies), complex64 [n_batch][n_f]
  *   h_power       HOST, float32 [n_batch][n_z][n_f]
  */
 fdas_status fdas_convolve_host(fdas_plan *plan, const void *h_spectrum, float *h_power, void *cuda_stream);
+
+/*
+ * The paper's general convolution ("produce the linear convolution", Table 2): the same path,
+ * but the filtered spectrum A' of eq.(2) itself is stored instead of its power.
+ *   d_amp         DEVICE, complex64 [n_batch][n_z][n_f], written completely, 8-byte aligned
+ * Otherwise as fdas_convolve (asynchronous, same errors).
+ */
+fdas_status fdas_convolve_complex(fdas_plan *plan, const void *d_spectrum, void *d_amp, void *cuda_stream);
+
+/*
+ * The hot path fused with the first step of detection ("detect"; "FDAS code"; the paper leaves the
+ * detection stage to Dimoudi et al. 2017, so this one is defined here, reading 17): the power plane is
+ * never written.  The columns are cut into n_blk = fdas_plan_nseg(plan) blocks of blk = fdas_plan_step(plan)
+ * columns, block s = [s*blk, min((s+1)*blk, n_f)), and for every batch item b, template row i and block s
+ *   d_max[b][i][s] = max over the block of P[b][i][r0]                  (float32, the value the plane would hold)
+ *   d_arg[b][i][s] = the smallest r0 - s*blk that attains it             (int32, 0 <= . < blk)
+ *   d_max, d_arg  DEVICE, [n_batch][n_z][n_blk], 4-byte aligned, written completely
+ * Comparisons are made on the float32 powers; equal powers resolve to the lowest column.  Deterministic.
+ * Otherwise as fdas_convolve (asynchronous, same errors).  fdas_detect_blockmax_host is the HOST-pointer
+ * convenience (spectrum in, the two small arrays out; synchronises the stream), like fdas_convolve_host.
+ */
+fdas_status fdas_detect_blockmax(fdas_plan *plan, const void *d_spectrum, float *d_max, int32_t *d_arg, void *cuda_stream);
+fdas_status fdas_detect_blockmax_host(fdas_plan *plan, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream);
 
 /* Free the plan and everything it owns.  NULL is accepted. */
 fdas_status fdas_plan_destroy(fdas_plan *plan);

@@ -22,6 +22,9 @@ SYMBOLS = {
     "fdas_set_templates": (_int, [_vp, _vp]),
     "fdas_convolve": (_int, [_vp, _vp, _vp, _vp]),
     "fdas_convolve_host": (_int, [_vp, _vp, _vp, _vp]),
+    "fdas_convolve_complex": (_int, [_vp, _vp, _vp, _vp]),
+    "fdas_detect_blockmax": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "fdas_detect_blockmax_host": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "fdas_plan_destroy": (_int, [_vp]),
     "fdas_plan_nz": (_int, [_vp]),
     "fdas_plan_step": (_int, [_vp]),
@@ -139,6 +142,19 @@ class Plan:
         """HOST buffers (pinned torch tensors or numpy arrays); copies are inside the call."""
         _check(lib().fdas_convolve_host(self._h, _ptr(h_spectrum), _ptr(h_power), _stream(stream)),
                "fdas_convolve_host")
+
+    def convolve_complex(self, d_spectrum, d_amp, stream=None):
+        """d_amp: DEVICE complex64 [n_batch][n_z][n_f], the filtered spectrum A' of eq.(2)."""
+        _check(lib().fdas_convolve_complex(self._h, _ptr(d_spectrum), _ptr(d_amp), _stream(stream)), "fdas_convolve_complex")
+
+    def detect_blockmax(self, d_spectrum, d_max, d_arg, stream=None):
+        """d_max float32, d_arg int32: DEVICE [n_batch][n_z][n_seg]; blocks of `step` columns."""
+        _check(lib().fdas_detect_blockmax(self._h, _ptr(d_spectrum), _ptr(d_max), _ptr(d_arg), _stream(stream)),
+               "fdas_detect_blockmax")
+
+    def detect_blockmax_host(self, h_spectrum, h_max, h_arg, stream=None):
+        _check(lib().fdas_detect_blockmax_host(self._h, _ptr(h_spectrum), _ptr(h_max), _ptr(h_arg), _stream(stream)),
+               "fdas_detect_blockmax_host")
 
     def destroy(self):
         if self._h:

@@ -209,9 +209,15 @@ __device__ __forceinline__ void forward_to_inv_layout(float2 *v, float2 *buf0, f
         }
 }
 
+// |y|^2 (a5) with the rounding spelled out, so that every output mode produces the same bits
+__device__ __forceinline__ float power_of(float2 y) { return __fmaf_rn(y.x, y.x, __fmul_rn(y.y, y.y)); }
+
 struct ConvParams {
     const float2 *__restrict__ spectrum; // [n_batch][n_f]
-    float *__restrict__ power;           // [n_batch][n_z][n_f]
+    float *__restrict__ power;           // OUT_POWER: [n_batch][n_z][n_f]
+    float2 *__restrict__ amp;            // OUT_AMP: [n_batch][n_z][n_f] complex A' (eq.(2) itself)
+    float *__restrict__ bmax;            // OUT_BLOCKMAX: [n_batch][n_z][n_seg] maximum power of the segment's columns
+    int *__restrict__ barg;              // OUT_BLOCKMAX: [n_batch][n_z][n_seg] lowest column offset attaining it
     const float4 *__restrict__ gperm;    // [n_z][E/2][NT] : template spectra in register order
     const float2 *__restrict__ tw;       // [L] : w_L^j
     unsigned int *__restrict__ work;     // [2] : next work item, CTAs finished (both 0 between launches)
@@ -224,6 +230,13 @@ struct ConvParams {
     int bulk_ok;                         // spectrum base is 16-byte aligned: interior segments may be bulk-copied
 };
 
+// What the kernel does with the filtered segment y_z (a5, a6):
+//   OUT_POWER     |y|^2 -> float32 power plane (BASELINE.json north_star)
+//   OUT_AMP       y itself -> complex64 plane: the paper's general convolution (Table 2)
+//   OUT_BLOCKMAX  max and argmax of |y|^2 over the segment's S columns: the plane never reaches HBM
+//                 (reading 17)
+enum { OUT_POWER = 0, OUT_AMP = 1, OUT_BLOCKMAX = 2 };
+
 template <class C> constexpr size_t conv_smem_bytes()
 {
     return 2 * sizeof(float2) * (size_t)InvCfg<C>::BUF_ELEMS + sizeof(float2) * (size_t)C::L;
@@ -233,7 +246,7 @@ template <class C> constexpr size_t conv_smem_bytes()
 // the tensor-memory budget); every CTA sets up its tensor-memory tables once and then takes
 // (batch item, segment) work items from a global counter until none is left.  Dynamic rather than
 // strided assignment because the CTAs sharing an SM do not run at the same speed (profiles/r1_c3_v5.md).
-template <int L>
+template <int L, int OUT>
 __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convolve_kernel(const ConvParams p)
 {
     using C = Cfg<L>;
@@ -249,6 +262,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     __shared__ __align__(8) uint64_t g_bar;
     __shared__ uint32_t tmem_slot;
     __shared__ uint32_t s_work[2];
+    __shared__ uint2 s_part[2][(Cfg<L>::NT + 31) / 32]; // OUT_BLOCKMAX: per-warp (power bits, position), by parity of z
 
     const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
 
@@ -294,6 +308,9 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     TwTmem<C> tws{tm_addr};
     uint32_t gphase = 0; // parity of the next completion of g_bar
     const bool fast_m = (p.m * 8 == L);
+    // OUT_AMP: the unit phase the static shuffle exchange leaves on this thread's outputs (fft_device.cuh)
+    float2 fix = make_float2(1.f, 0.f);
+    if constexpr (OUT == OUT_AMP) fix = __ldg(p.tw + inv_fix_index<C>(t));
 
     // a1 through the bulk-copy engine: segment `w` can be copied as one 16-byte aligned block of L
     // complex64 if it lies inside [0, n_f); the first and last segment(s) need the zero padding of
@@ -353,6 +370,8 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
 
         const int64_t col0 = seg * p.S - p.m + t;                             // column of y[t]
         float *__restrict__ out = p.power + bi * p.n_z * p.n_f + col0;        // row 0 of this batch item
+        float2 *__restrict__ out_c = p.amp + bi * p.n_z * p.n_f + col0;
+        int64_t bm_idx = (bi * p.n_z) * p.n_seg + seg;                         // OUT_BLOCKMAX: entry of row 0
         const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
         const bool fast8 = interior && fast_m;
         const bool fast = interior && (p.m % NT == 0) && (p.m / NT <= 4);
@@ -397,39 +416,97 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
         // reads, 1/3 of the arithmetic) sits between the exchange write of template z and its barrier, so
         // a warp that reaches the barrier early has independent work instead of idling.  The loop exists
         // once per store mode (a5 + a6 below) so that the mode costs nothing inside it.
+        // OUT_BLOCKMAX: block result of template zz from the per-warp partials (one warp, after a barrier)
+        auto finalize_max = [&](int zz) {
+            if (warp == 0) {
+                constexpr int NW = (NT + 31) / 32;
+                const uint2 pr = lane < NW ? s_part[zz & 1][lane] : make_uint2(0u, 0x7fffffffu);
+                const unsigned wm = __reduce_max_sync(0xffffffffu, pr.x);
+                const unsigned wc = __reduce_min_sync(0xffffffffu, pr.x == wm ? pr.y : 0x7fffffffu);
+                if (lane == 0) {
+                    const int64_t o = bm_idx + (int64_t)zz * p.n_seg;
+                    p.bmax[o] = __uint_as_float(wm);
+                    p.barg[o] = (int)wc - p.m;
+                }
+            }
+        };
         auto z_loop = [&](auto mode_tag) {
             constexpr int MODE = decltype(mode_tag)::value;
+            // which registers are outputs of this segment: u[d] is y[d*NT + t], kept if m <= d*NT + t < m + S
+            // and its column exists.  MODE 0: interior segment and m = L/8; MODE 1: interior segment and m a
+            // small multiple of the thread count; MODE 2: anything else, per-element bounds.
+            auto kept = [&](int d) -> bool {
+                if constexpr (MODE == 0) return d >= D0_FAST;
+                else if constexpr (MODE == 1) return d >= 4 || d >= d0;
+                else {
+                    const int pidx = d * NT + t;
+                    return pidx >= p.m && pidx < p.m + p.S && col0 + d * NT < p.n_f;
+                }
+            };
             for (int z = 0; z < p.n_z; ++z) {
                 float2 *bufa = (C::P == 3 && (z & 1)) ? buf1 : buf0;
                 inv_stage_b<C>(v, bufa, A, tws, lane);
                 if (z + 1 < p.n_z) stage_a();
                 __syncthreads();
                 fetch_slot(z + 2);
+                if constexpr (OUT == OUT_BLOCKMAX) {
+                    if (z > 0) finalize_max(z - 1);
+                }
                 float2 u[E];
                 inv_stage_c<C>(u, bufa, buf1, A, tw0, tws);
-                // a5 + a6: trim, power, coalesced store
-                if constexpr (MODE == 0) {        // interior segment, m = L/8: registers D0_FAST.. are kept
-#pragma unroll
-                    for (int d = D0_FAST; d < E; ++d) __stcs(out + d * NT, u[d].x * u[d].x + u[d].y * u[d].y);
-                } else if constexpr (MODE == 1) { // interior segment, m a small multiple of the thread count
+                // a5 + a6: trim, then power / amplitude / block maximum
+                if constexpr (OUT == OUT_POWER) {
 #pragma unroll
                     for (int d = 0; d < E; ++d) {
-                        if (d >= 4 || d >= d0) __stcs(out + d * NT, u[d].x * u[d].x + u[d].y * u[d].y);
+                        if (MODE == 0 && d < D0_FAST) continue;
+                        if (kept(d)) {
+                            const float pw = power_of(u[d]);
+                            if constexpr (MODE == 2) out[d * NT] = pw;
+                            else __stcs(out + d * NT, pw);
+                        }
                     }
-                } else {                          // anything else: per-element bounds
+                    out += p.n_f;
+                } else if constexpr (OUT == OUT_AMP) {
 #pragma unroll
                     for (int d = 0; d < E; ++d) {
-                        const int pidx = d * NT + t;
-                        const int64_t col = col0 + d * NT;
-                        if (pidx >= p.m && pidx < p.m + p.S && col < p.n_f) out[d * NT] = u[d].x * u[d].x + u[d].y * u[d].y;
+                        if (MODE == 0 && d < D0_FAST) continue;
+                        if (kept(d)) {
+                            const float2 a = cmul(u[d], fix);
+                            if constexpr (MODE == 2) out_c[d * NT] = a;
+                            else __stcs(out_c + d * NT, a);
+                        }
                     }
+                    out_c += p.n_f;
+                } else {
+                    float pw[E];
+                    float best = 0.f; // powers are >= 0, so their bit patterns order like unsigned integers
+#pragma unroll
+                    for (int d = 0; d < E; ++d) {
+                        pw[d] = power_of(u[d]);
+                        if (MODE == 0 && d < D0_FAST) continue;
+                        if (kept(d)) best = fmaxf(best, pw[d]);
+                    }
+                    const unsigned wm = __reduce_max_sync(0xffffffffu, __float_as_uint(best));
+                    unsigned pos = 0x7fffffffu;
+                    if (__float_as_uint(best) == wm) { // rare: the lanes that hold the warp's maximum look up where
+#pragma unroll
+                        for (int d = E - 1; d >= 0; --d) {
+                            if (MODE == 0 && d < D0_FAST) continue;
+                            if (kept(d) && __float_as_uint(pw[d]) == wm) pos = (unsigned)(d * NT + t);
+                        }
+                    }
+                    const unsigned wp = __reduce_min_sync(0xffffffffu, pos);
+                    if (lane == 0) s_part[z & 1][warp] = make_uint2(wm, wp);
                 }
-                out += p.n_f;
             }
         };
         if (fast8) z_loop(std::integral_constant<int, 0>{});
         else if (fast) z_loop(std::integral_constant<int, 1>{});
         else z_loop(std::integral_constant<int, 2>{});
+        if constexpr (OUT == OUT_BLOCKMAX) {
+            __syncthreads();
+            finalize_max(p.n_z - 1);
+        }
         slot ^= 1;
         w = s_work[slot];
     }

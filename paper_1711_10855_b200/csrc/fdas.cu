@@ -122,13 +122,14 @@ struct fdas_plan {
     int last_cuda_error;
     int last_launches;
     int device;               // CUDA device the plan lives on (every call checks it)
-    int grid_max;             // resident CTAs of the hot kernel on this device (registers, smem, tensor memory)
+    int grid_max[3];          // resident CTAs of the hot kernel per output mode (registers, smem, tensor memory)
     unsigned int *d_work;     // [WORK_SLOTS][2] work counters of the persistent kernel, zero between launches
     unsigned int work_seq;    // launches so far: selects the counter pair
     // buffers of fdas_convolve_host
     void *d_host_spec;
     float *d_host_power;
-    size_t host_spec_bytes, host_power_bytes;
+    void *d_host_det;
+    size_t host_spec_bytes, host_power_bytes, host_det_bytes;
 };
 
 namespace {
@@ -173,9 +174,9 @@ template <int L> size_t smem_bytes() { return 2 * sizeof(float2) * (size_t)InvCf
 // that run concurrently (several streams) use different pairs; a pair is re-armed by its own launch.
 constexpr unsigned WORK_SLOTS = 1024;
 
-template <int L> cudaError_t launch_convolve(const ConvParams &cp, int grid_max, cudaStream_t st)
+template <int L, int OUT> cudaError_t launch_convolve(const ConvParams &cp, int grid_max, cudaStream_t st)
 {
-    auto kern = fdas_convolve_kernel<L>;
+    auto kern = fdas_convolve_kernel<L, OUT>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
     if (cp.n_work > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const unsigned grid = (unsigned)(cp.n_work < grid_max ? cp.n_work : grid_max);
@@ -187,9 +188,9 @@ template <int L> cudaError_t launch_convolve(const ConvParams &cp, int grid_max,
 // memory and size the persistent grid = resident CTAs per SM x SMs.  Resident CTAs are counted here
 // from the kernel's registers and shared memory, the SM's thread / block limits and the tensor memory
 // (512 columns per SM); the occupancy API reports one CTA per SM for a kernel that allocates tensor memory.
-template <int L> cudaError_t prepare_convolve(int device, int *grid_max)
+template <int L, int OUT> cudaError_t prepare_convolve(int device, int *grid_max)
 {
-    auto kern = fdas_convolve_kernel<L>;
+    auto kern = fdas_convolve_kernel<L, OUT>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
     constexpr int NT = Cfg<L>::NT;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -317,7 +318,9 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
     if (e == cudaSuccess) e = cudaMemset(p->d_work, 0, sizeof(unsigned int) * 2 * WORK_SLOTS);
     if (e == cudaSuccess) {
         const int L = p->L;
-        FDAS_DISPATCH_L(L, e = prepare_convolve<LL>(p->device, &p->grid_max));
+        FDAS_DISPATCH_L(L, (e = prepare_convolve<LL, OUT_POWER>(p->device, &p->grid_max[OUT_POWER])));
+        if (e == cudaSuccess) { FDAS_DISPATCH_L(L, (e = prepare_convolve<LL, OUT_AMP>(p->device, &p->grid_max[OUT_AMP]))); }
+        if (e == cudaSuccess) { FDAS_DISPATCH_L(L, (e = prepare_convolve<LL, OUT_BLOCKMAX>(p->device, &p->grid_max[OUT_BLOCKMAX]))); }
     }
     if (e != cudaSuccess) {
         fdas_status s = (e == cudaErrorMemoryAllocation) ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
@@ -362,15 +365,18 @@ fdas_status fdas_set_templates(fdas_plan *p, const float *h_templates)
     return FDAS_OK;
 }
 
-fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, void *cuda_stream)
+// common part of the three entry points that enqueue the hot kernel
+static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, float *d_power, float2 *d_amp,
+                           float *d_max, int *d_arg, void *cuda_stream)
 {
-    if (!p || !d_spectrum || !d_power) return FDAS_ERR_INVALID_ARG;
-    if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_power & 3u)) return FDAS_ERR_INVALID_ARG;
     if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
     ConvParams cp;
     cp.spectrum = (const float2 *)d_spectrum;
     cp.power = d_power;
+    cp.amp = d_amp;
+    cp.bmax = d_max;
+    cp.barg = d_arg;
     cp.gperm = p->d_gperm;
     cp.tw = p->d_tw;
     cp.work = p->d_work + 2 * (p->work_seq++ % WORK_SLOTS);
@@ -384,39 +390,90 @@ fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
-    FDAS_DISPATCH_L(L, (e = launch_convolve<LL>(cp, p->grid_max, st)));
+    switch (out_mode) {
+    case OUT_POWER: FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_POWER>(cp, p->grid_max[OUT_POWER], st))); break;
+    case OUT_AMP: FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_AMP>(cp, p->grid_max[OUT_AMP], st))); break;
+    case OUT_BLOCKMAX: FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_BLOCKMAX>(cp, p->grid_max[OUT_BLOCKMAX], st))); break;
+    default: break;
+    }
     p->last_launches = 1;
     if (e != cudaSuccess) return cuda_fail(p, e);
     return FDAS_OK;
 }
 
+fdas_status fdas_convolve(fdas_plan *p, const void *d_spectrum, float *d_power, void *cuda_stream)
+{
+    if (!p || !d_spectrum || !d_power) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_power & 3u)) return FDAS_ERR_INVALID_ARG;
+    return enqueue(p, OUT_POWER, d_spectrum, d_power, nullptr, nullptr, nullptr, cuda_stream);
+}
+
+fdas_status fdas_convolve_complex(fdas_plan *p, const void *d_spectrum, void *d_amp, void *cuda_stream)
+{
+    if (!p || !d_spectrum || !d_amp) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_amp & 7u)) return FDAS_ERR_INVALID_ARG;
+    return enqueue(p, OUT_AMP, d_spectrum, nullptr, (float2 *)d_amp, nullptr, nullptr, cuda_stream);
+}
+
+fdas_status fdas_detect_blockmax(fdas_plan *p, const void *d_spectrum, float *d_max, int32_t *d_arg, void *cuda_stream)
+{
+    if (!p || !d_spectrum || !d_max || !d_arg) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_max & 3u) || ((uintptr_t)d_arg & 3u)) return FDAS_ERR_INVALID_ARG;
+    return enqueue(p, OUT_BLOCKMAX, d_spectrum, nullptr, nullptr, d_max, (int *)d_arg, cuda_stream);
+}
+
+// plan-owned staging buffers of the *_host entry points: grown on demand, kept until destroy
+static cudaError_t stage_reserve(void **buf, size_t *have, size_t need)
+{
+    if (*have >= need) return cudaSuccess;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr;
+    *have = 0;
+    cudaError_t e = cudaMalloc(buf, need);
+    if (e == cudaSuccess) *have = need;
+    return e;
+}
+
 fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_power, void *cuda_stream)
 {
     if (!p || !h_spectrum || !h_power) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
     const size_t sb = sizeof(float2) * (size_t)p->n_batch * (size_t)p->n_f;
     const size_t pb = sizeof(float) * (size_t)p->n_batch * (size_t)p->n_z * (size_t)p->n_f;
-    cudaError_t e = cudaSuccess;
-    if (p->host_spec_bytes < sb) {
-        if (p->d_host_spec) cudaFree(p->d_host_spec);
-        p->d_host_spec = nullptr; p->host_spec_bytes = 0;
-        e = cudaMalloc(&p->d_host_spec, sb);
-        if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
-        p->host_spec_bytes = sb;
-    }
-    if (p->host_power_bytes < pb) {
-        if (p->d_host_power) cudaFree(p->d_host_power);
-        p->d_host_power = nullptr; p->host_power_bytes = 0;
-        e = cudaMalloc((void **)&p->d_host_power, pb);
-        if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
-        p->host_power_bytes = pb;
-    }
+    cudaError_t e = stage_reserve(&p->d_host_spec, &p->host_spec_bytes, sb);
+    if (e == cudaSuccess) e = stage_reserve((void **)&p->d_host_power, &p->host_power_bytes, pb);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(p, e);
     fdas_status s = fdas_convolve(p, p->d_host_spec, p->d_host_power, cuda_stream);
     if (s != FDAS_OK) return s;
     e = cudaMemcpyAsync(h_power, p->d_host_power, pb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return FDAS_OK;
+}
+
+fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream)
+{
+    if (!p || !h_spectrum || !h_max || !h_arg) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
+    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
+    const size_t sb = sizeof(float2) * (size_t)p->n_batch * (size_t)p->n_f;
+    const size_t nb = (size_t)p->n_batch * (size_t)p->n_z * (size_t)p->n_seg; // entries of each result array
+    cudaError_t e = stage_reserve(&p->d_host_spec, &p->host_spec_bytes, sb);
+    if (e == cudaSuccess) e = stage_reserve(&p->d_host_det, &p->host_det_bytes, 8 * nb);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+    float *d_max = (float *)p->d_host_det;
+    int32_t *d_arg = (int32_t *)p->d_host_det + nb;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    fdas_status s = fdas_detect_blockmax(p, p->d_host_spec, d_max, d_arg, cuda_stream);
+    if (s != FDAS_OK) return s;
+    e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(p, e);
     return FDAS_OK;
@@ -430,6 +487,7 @@ fdas_status fdas_plan_destroy(fdas_plan *p)
     if (p->d_work) cudaFree(p->d_work);
     if (p->d_host_spec) cudaFree(p->d_host_spec);
     if (p->d_host_power) cudaFree(p->d_host_power);
+    if (p->d_host_det) cudaFree(p->d_host_det);
     (void)cudaGetLastError();
     free(p);
     return FDAS_OK;
@@ -439,7 +497,7 @@ int fdas_plan_nz(const fdas_plan *p) { return p ? p->n_z : 0; }
 int fdas_plan_step(const fdas_plan *p) { return p ? p->S : 0; }
 int64_t fdas_plan_nseg(const fdas_plan *p) { return p ? p->n_seg : 0; }
 int fdas_plan_batch(const fdas_plan *p) { return p ? p->n_batch : 0; }
-int fdas_plan_grid(const fdas_plan *p) { return p ? p->grid_max : 0; }
+int fdas_plan_grid(const fdas_plan *p) { return p ? p->grid_max[OUT_POWER] : 0; }
 int fdas_plan_last_launch_count(const fdas_plan *p) { return p ? p->last_launches : 0; }
 int fdas_plan_last_cuda_error(const fdas_plan *p) { return p ? p->last_cuda_error : -1; }
 
