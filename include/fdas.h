@@ -131,6 +131,29 @@ fdas_status fdas_convolve_complex(fdas_plan *plan, const void *d_spectrum, void 
 fdas_status fdas_detect_blockmax(fdas_plan *plan, const void *d_spectrum, float *d_max, int32_t *d_arg, void *cuda_stream);
 fdas_status fdas_detect_blockmax_host(fdas_plan *plan, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream);
 
+/*
+ * The segment FFT as a stand-alone batched transform (eq.(3); the stand-alone comparison of P:46 and
+ * Table 1: "100 FFTs per kernel launch, while launching 1000 of these kernels", N = 1024, with the
+ * number of elements per thread as the design axis).  Same device code as the convolution kernel's forward
+ * transform; natural order in and out.
+ *   n                 512, 1024, 2048, 4096 or 8192 (else FDAS_ERR_UNSUPPORTED)
+ *   elems_per_thread  0 = the convolution kernel's choice; 8 (n = 512, 1024) or 16 (n >= 1024); other
+ *                     combinations are FDAS_ERR_UNSUPPORTED
+ * fdas_fft_exec enqueues one launch that transforms n_fft contiguous sequences:
+ *   d_in, d_out       DEVICE, complex64 [n_fft][n], 8-byte aligned, must not overlap
+ *   inverse           0: eq.(3);  1: the unnormalised inverse (conjugate twiddles)
+ * Asynchronous; never allocates or synchronises.  Errors as fdas_convolve.
+ */
+typedef struct fdas_fft_plan fdas_fft_plan;
+fdas_status fdas_fft_plan_create(fdas_fft_plan **out, int n, int elems_per_thread);
+fdas_status fdas_fft_exec(fdas_fft_plan *plan, int64_t n_fft, const void *d_in, void *d_out, int inverse, void *cuda_stream);
+/* The repetition scheme of P:46: n_launches identical launches of n_fft transforms each, enqueued back to back. */
+fdas_status fdas_fft_exec_many(fdas_fft_plan *plan, int n_launches, int64_t n_fft, const void *d_in, void *d_out,
+                               int inverse, void *cuda_stream);
+fdas_status fdas_fft_plan_destroy(fdas_fft_plan *plan);
+int fdas_fft_plan_elems_per_thread(const fdas_fft_plan *plan);
+int fdas_fft_plan_grid(const fdas_fft_plan *plan);   /* CTAs of one launch at most (grid-stride over the batch) */
+
 /* Free the plan and everything it owns.  NULL is accepted. */
 fdas_status fdas_plan_destroy(fdas_plan *plan);
 

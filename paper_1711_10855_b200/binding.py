@@ -34,6 +34,12 @@ SYMBOLS = {
     "fdas_plan_last_launch_count": (_int, [_vp]),
     "fdas_plan_last_cuda_error": (_int, [_vp]),
     "fdas_status_string": (ctypes.c_char_p, [_int]),
+    "fdas_fft_plan_create": (_int, [ctypes.POINTER(_vp), _int, _int]),
+    "fdas_fft_exec": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
+    "fdas_fft_exec_many": (_int, [_vp, _int, _i64, _vp, _vp, _int, _vp]),
+    "fdas_fft_plan_destroy": (_int, [_vp]),
+    "fdas_fft_plan_elems_per_thread": (_int, [_vp]),
+    "fdas_fft_plan_grid": (_int, [_vp]),
     "fdas_debug_fft": (_int, [_int, _i64, _vp, _vp, _int]),
     "fdas_debug_layout": (_i64, [_int, _int, _int, _int, _int]),
     "fdas_version": (ctypes.c_char_p, []),
@@ -159,6 +165,39 @@ class Plan:
     def destroy(self):
         if self._h:
             lib().fdas_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class FftPlan:
+    """fdas_fft_plan_create ... fdas_fft_plan_destroy: the stand-alone batched segment FFT."""
+
+    def __init__(self, n, elems_per_thread=0):
+        self._h = _vp()
+        _check(lib().fdas_fft_plan_create(ctypes.byref(self._h), int(n), int(elems_per_thread)), "fdas_fft_plan_create")
+        self.n = int(n)
+
+    @property
+    def elems_per_thread(self): return lib().fdas_fft_plan_elems_per_thread(self._h)
+    @property
+    def grid(self): return lib().fdas_fft_plan_grid(self._h)
+
+    def exec(self, n_fft, d_in, d_out, inverse=False, stream=None):
+        _check(lib().fdas_fft_exec(self._h, int(n_fft), _ptr(d_in), _ptr(d_out), int(bool(inverse)), _stream(stream)),
+               "fdas_fft_exec")
+
+    def exec_many(self, n_launches, n_fft, d_in, d_out, inverse=False, stream=None):
+        _check(lib().fdas_fft_exec_many(self._h, int(n_launches), int(n_fft), _ptr(d_in), _ptr(d_out), int(bool(inverse)),
+                                        _stream(stream)), "fdas_fft_exec_many")
+
+    def destroy(self):
+        if self._h:
+            lib().fdas_fft_plan_destroy(self._h)
             self._h = _vp()
 
     def __del__(self):

@@ -18,6 +18,7 @@
 #include "../../include/fdas.h"
 #include "fft_device.cuh"
 #include "convolve.cuh"
+#include "fft_batch.cuh"
 
 namespace fdas {
 
@@ -290,6 +291,44 @@ template <int L> static int64_t layout_query(int what, int t, int a, int b)
     }
 }
 
+// -------------------------------------------------------------------------------------------
+// stand-alone batched FFT (NEXT-4; Table 1)
+// -------------------------------------------------------------------------------------------
+struct fdas_fft_plan {
+    int n, e, device, grid_max;
+    float2 *d_tw;
+};
+
+template <class C> static cudaError_t fft_batch_prepare(int device, int *grid_max)
+{
+    auto kern = fdas_fft_batch_kernel<C>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_batch_smem_bytes<C>());
+    if (e != cudaSuccess) return e;
+    int per_sm = 0, n_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::NT, fft_batch_smem_bytes<C>());
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    *grid_max = per_sm * n_sm;
+    return cudaSuccess;
+}
+template <class C> static cudaError_t fft_batch_launch(const fdas_fft_plan *p, int64_t n_fft, const float2 *in, float2 *out,
+                                                       int inverse, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)(n_fft < p->grid_max ? n_fft : p->grid_max);
+    fdas_fft_batch_kernel<C><<<grid, C::NT, fft_batch_smem_bytes<C>(), st>>>(in, out, p->d_tw, (long long)n_fft, inverse);
+    return cudaGetLastError();
+}
+// (n, elements per thread) -> kernel configuration
+#define FDAS_DISPATCH_FFT(N, E, EXPR)                                              \
+    if ((N) == 512 && (E) == 8) { using CC = Cfg<512>; EXPR; }                     \
+    else if ((N) == 1024 && (E) == 8) { using CC = Cfg1024E8; EXPR; }              \
+    else if ((N) == 1024 && (E) == 16) { using CC = Cfg<1024>; EXPR; }             \
+    else if ((N) == 2048 && (E) == 16) { using CC = Cfg<2048>; EXPR; }             \
+    else if ((N) == 4096 && (E) == 16) { using CC = Cfg<4096>; EXPR; }             \
+    else if ((N) == 8192 && (E) == 16) { using CC = Cfg<8192>; EXPR; }
+
 extern "C" {
 
 fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step, int template_width, int segment_len)
@@ -500,6 +539,66 @@ int fdas_plan_batch(const fdas_plan *p) { return p ? p->n_batch : 0; }
 int fdas_plan_grid(const fdas_plan *p) { return p ? p->grid_max[OUT_POWER] : 0; }
 int fdas_plan_last_launch_count(const fdas_plan *p) { return p ? p->last_launches : 0; }
 int fdas_plan_last_cuda_error(const fdas_plan *p) { return p ? p->last_cuda_error : -1; }
+
+fdas_status fdas_fft_plan_create(fdas_fft_plan **out, int n, int elems_per_thread)
+{
+    if (!out) return FDAS_ERR_INVALID_ARG;
+    if (!supported_L(n)) return FDAS_ERR_UNSUPPORTED;
+    int e_thr = elems_per_thread ? elems_per_thread : (n == 512 ? 8 : 16);
+    if (!((e_thr == 8 && (n == 512 || n == 1024)) || (e_thr == 16 && n >= 1024))) return FDAS_ERR_UNSUPPORTED;
+    fdas_fft_plan *p = (fdas_fft_plan *)calloc(1, sizeof(fdas_fft_plan));
+    if (!p) return FDAS_ERR_ALLOC;
+    p->n = n;
+    p->e = e_thr;
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = upload_twiddles(n, &p->d_tw);
+    if (e == cudaSuccess) { FDAS_DISPATCH_FFT(n, e_thr, (e = fft_batch_prepare<CC>(p->device, &p->grid_max))) }
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (p->d_tw) cudaFree(p->d_tw);
+        free(p);
+        return e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+fdas_status fdas_fft_exec(fdas_fft_plan *p, int64_t n_fft, const void *d_in, void *d_out, int inverse, void *cuda_stream)
+{
+    if (!p || !d_in || !d_out || n_fft < 0 || d_in == d_out) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in & 7u) || ((uintptr_t)d_out & 7u)) return FDAS_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return FDAS_ERR_INVALID_ARG;
+    if (n_fft == 0) return FDAS_OK;
+    cudaError_t e = cudaErrorInvalidValue;
+    FDAS_DISPATCH_FFT(p->n, p->e, (e = fft_batch_launch<CC>(p, n_fft, (const float2 *)d_in, (float2 *)d_out, inverse,
+                                                            (cudaStream_t)cuda_stream)))
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    return FDAS_OK;
+}
+
+fdas_status fdas_fft_exec_many(fdas_fft_plan *p, int n_launches, int64_t n_fft, const void *d_in, void *d_out, int inverse,
+                               void *cuda_stream)
+{
+    if (n_launches < 0) return FDAS_ERR_INVALID_ARG;
+    for (int i = 0; i < n_launches; ++i) {
+        fdas_status s = fdas_fft_exec(p, n_fft, d_in, d_out, inverse, cuda_stream);
+        if (s != FDAS_OK) return s;
+    }
+    return FDAS_OK;
+}
+
+fdas_status fdas_fft_plan_destroy(fdas_fft_plan *p)
+{
+    if (!p) return FDAS_OK;
+    if (p->d_tw) cudaFree(p->d_tw);
+    (void)cudaGetLastError();
+    free(p);
+    return FDAS_OK;
+}
+
+int fdas_fft_plan_elems_per_thread(const fdas_fft_plan *p) { return p ? p->e : 0; }
+int fdas_fft_plan_grid(const fdas_fft_plan *p) { return p ? p->grid_max : 0; }
 
 const char *fdas_status_string(fdas_status s)
 {

@@ -50,6 +50,9 @@ template <> struct Cfg<1024> : CfgT<1024, 16, 16, 8, 8, 1> {};
 template <> struct Cfg<2048> : CfgT<2048, 16, 16, 16, 8, 1> {};
 template <> struct Cfg<4096> : CfgT<4096, 16, 16, 16, 16, 1> {};
 template <> struct Cfg<8192> : CfgT<8192, 16, 16, 8, 8, 8> {};
+// N = 1024 with 8 elements per thread (forward passes only: the stand-alone FFT of P:46, Table 1, whose design
+// axis is the number of elements per thread; the convolution kernel uses Cfg<1024> with 16)
+struct Cfg1024E8 : CfgT<1024, 8, 8, 8, 8, 2> {};
 
 // ---------------------------------------------------------------------------------------------
 // complex helpers

@@ -27,3 +27,58 @@ def test_segment_fft_vs_oracle(oracle, L, inverse):
     k = np.arange(L)
     tone = np.exp(sign * 2j * np.pi * k / L)
     assert np.max(np.abs(y[1] - tone)) < 1e-5
+
+
+@pytest.mark.parametrize("n,e", [(512, 8), (1024, 8), (1024, 16), (2048, 16), (4096, 16), (8192, 16)])
+@pytest.mark.parametrize("inverse", [False, True])
+def test_batched_fft_vs_oracle(oracle, n, e, inverse):
+    """fdas_fft_exec (the stand-alone FFT of P:46 / Table 1; elements per thread is its design axis) on a batch
+    that is not a multiple of anything, natural order in and out, both directions."""
+    import torch
+    from paper_1711_10855_b200 import binding
+    rng = np.random.default_rng(n + e + int(inverse))
+    n_fft = 301
+    x = (rng.standard_normal((n_fft, n)) + 1j * rng.standard_normal((n_fft, n))).astype(np.complex64)
+    x[1] = 0; x[1, 1] = 1.0
+    x[2] = 0; x[2, n - 1] = 1.0j
+    plan = binding.FftPlan(n, e)
+    assert plan.elems_per_thread == e and plan.grid >= 148
+    d_in = torch.from_numpy(x).cuda()
+    d_out = torch.full_like(d_in, float("nan"))
+    plan.exec(n_fft, d_in, d_out, inverse=inverse)
+    torch.cuda.synchronize()
+    y = d_out.cpu().numpy()
+    assert np.all(np.isfinite(y.view(np.float32)))
+    sign = +1 if inverse else -1
+    for s in (0, 1, 2, 147, 148, 300):
+        ref = oracle.fft(x[s].astype(np.complex128), sign=sign)
+        scale = np.sqrt(n) * np.abs(x[s]).max()
+        assert np.max(np.abs(y[s] - ref)) <= 2e-6 * scale * np.log2(n), (n, e, inverse, s)
+    # Parseval on every sequence (eq.(3) is unnormalised: sum |X|^2 = n sum |x|^2)
+    ex = (np.abs(x.astype(np.complex128)) ** 2).sum(axis=1)
+    ey = (np.abs(y.astype(np.complex128)) ** 2).sum(axis=1)
+    assert np.max(np.abs(ey / (n * ex) - 1.0)) < 1e-5
+    # inverse(forward(x)) = n x
+    d_back = torch.empty_like(d_in)
+    plan.exec(n_fft, d_out, d_back, inverse=not inverse)
+    torch.cuda.synchronize()
+    assert np.max(np.abs(d_back.cpu().numpy() / n - x)) < 2e-5
+    plan.destroy()
+
+
+def test_batched_fft_arguments():
+    import torch
+    from paper_1711_10855_b200 import binding
+    with pytest.raises(binding.FdasError) as ei:
+        binding.FftPlan(1000, 0)
+    assert ei.value.status == binding.FDAS_ERR_UNSUPPORTED
+    with pytest.raises(binding.FdasError) as ei:
+        binding.FftPlan(4096, 8)
+    assert ei.value.status == binding.FDAS_ERR_UNSUPPORTED
+    plan = binding.FftPlan(1024)
+    assert plan.elems_per_thread == 16
+    buf = torch.zeros((4, 1024), dtype=torch.complex64, device="cuda")
+    with pytest.raises(binding.FdasError):
+        plan.exec(4, buf, buf)              # in place is not supported
+    plan.exec(0, buf, torch.empty_like(buf))  # empty batch: nothing to do
+    plan.destroy()
