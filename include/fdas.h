@@ -82,6 +82,19 @@ fdas_status fdas_plan_set_batch(fdas_plan *plan, int n_batch);
 fdas_status fdas_set_templates(fdas_plan *plan, const float *h_templates);
 
 /*
+ * The FDAS-specific optimisation the paper mentions ("exploit symmetries in FDAS algorithm"): the
+ * response of trial -z is the complex conjugate of the response of +z, so P[-z](A) = P[+z](conj A) and one
+ * template fetch can serve two rows (SURVEY.md 8(c) note S).  enable != 0 asks
+ * fdas_convolve to use that form WHEN it is exact: fdas_set_templates checks that row n_z-1-i of the bank is the
+ * element-wise conjugate of row i bit for bit (n_z odd); any other bank, and segment lengths other than 2048 and
+ * 4096, silently take the general path.  Off by default: measured slower than the general path on
+ * BASELINE.json config 3 (profiles/r2_symmetry.md).  fdas_plan_symmetry_active tells which path the next
+ * fdas_convolve takes.  The result is the same to rounding (tests/test_gpu_symmetry.py).
+ */
+fdas_status fdas_plan_set_symmetry(fdas_plan *plan, int enable);
+int fdas_plan_symmetry_active(const fdas_plan *plan);
+
+/*
  * Enqueue the hot path on cuda_stream: for every batch item, segment and trial z -- segment load,
  * forward FFT (once per segment), pointwise multiply, inverse FFT, trim, |.|^2, power-plane write.
  *   d_spectrum    DEVICE, complex64 [n_batch][n_f], read only, 8-byte aligned

@@ -20,6 +20,8 @@ SYMBOLS = {
     "fdas_plan_create": (_int, [ctypes.POINTER(_vp), _i64, _int, _int, _int, _int]),
     "fdas_plan_set_batch": (_int, [_vp, _int]),
     "fdas_set_templates": (_int, [_vp, _vp]),
+    "fdas_plan_set_symmetry": (_int, [_vp, _int]),
+    "fdas_plan_symmetry_active": (_int, [_vp]),
     "fdas_convolve": (_int, [_vp, _vp, _vp, _vp]),
     "fdas_convolve_host": (_int, [_vp, _vp, _vp, _vp]),
     "fdas_convolve_complex": (_int, [_vp, _vp, _vp, _vp]),
@@ -132,6 +134,12 @@ class Plan:
 
     def set_batch(self, n_batch):
         _check(lib().fdas_plan_set_batch(self._h, int(n_batch)), "fdas_plan_set_batch")
+
+    def set_symmetry(self, enable):
+        _check(lib().fdas_plan_set_symmetry(self._h, int(bool(enable))), "fdas_plan_set_symmetry")
+
+    @property
+    def symmetry_active(self): return bool(lib().fdas_plan_symmetry_active(self._h))
 
     def set_templates(self, h_templates):
         """h_templates: complex64 [n_z][m] numpy array (HOST)."""

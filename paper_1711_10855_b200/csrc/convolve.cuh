@@ -246,7 +246,11 @@ template <class C> constexpr size_t conv_smem_bytes()
 // the tensor-memory budget); every CTA sets up its tensor-memory tables once and then takes
 // (batch item, segment) work items from a global counter until none is left.  Dynamic rather than
 // strided assignment because the CTAs sharing an SM do not run at the same speed (profiles/r1_c3_v5.md).
-template <int L, int OUT>
+// SYM ("FDAS specific ... symmetries"): the bank satisfies h_{-z} = conj(h_{+z})
+// (checked by fdas_set_templates).  Then P[-z](A) = P[+z](conj A) exactly, i.e. row -z is the same template
+// applied to DFT(conj x)[n] = conj(X[-n]), which is parked in tensor memory next to X: one template fetch
+// serves two rows.  The shortcut G_{-z} = conj(G_{+z}) is NOT exact for an even window and is not used.
+template <int L, int OUT, bool SYM = false>
 __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convolve_kernel(const ConvParams p)
 {
     using C = Cfg<L>;
@@ -255,6 +259,8 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     constexpr int E = C::E, NT = C::NT;
     constexpr uint32_t G_BYTES = (uint32_t)L * 8u;
     constexpr int D0_FAST = E / 8;       // first kept register when m = L/8 (every BASELINE.json config)
+    constexpr int XC_OFF = TC::TWM_OFF;  // SYM: DFT(conj x) sits in the column block that four-pass plans use for twiddles
+    static_assert(!SYM || (C::P == 3 && TC::TW0_PARKED && OUT == OUT_POWER), "SYM needs the free 32-column block");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *buf0 = reinterpret_cast<float2 *>(smem_raw);
     float2 *buf1 = buf0 + I::BUF_ELEMS;
@@ -366,10 +372,33 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
         forward_to_inv_layout<C, true>(v, buf0, buf1, p.tw, t);
         ptx::tmem_st16(tm_addr + TC::X_OFF, v);
         if constexpr (E > 8) ptx::tmem_st16(tm_addr + TC::X_OFF + 16, v + 8);
+        if constexpr (SYM) { // DFT(conj x)[f] = conj(X[-f]) from the natural-order copy the re-layout left in buf0
+            float2 xc[E];
+#pragma unroll
+            for (int i = 0; i < I::NB; ++i)
+#pragma unroll
+                for (int k = 0; k < I::Ra; ++k) {
+                    const int f = (L - inv_freq<C>(t, i, k)) & (L - 1);
+                    const float2 a = buf0[f + (f >> 4)];
+                    xc[i * I::Ra + k] = make_float2(a.x, -a.y);
+                }
+            ptx::tmem_st16(tm_addr + XC_OFF, xc);
+            if constexpr (E > 8) ptx::tmem_st16(tm_addr + XC_OFF + 16, xc + 8);
+        }
         ptx::tmem_wait_st();
+
+        // The z loop runs n_z iterations.  Iteration k: template G_{g(k)} on X (sel 0) or on DFT(conj x) (sel 1)
+        // produces row r(k).  Without SYM g = r = k.  With SYM the rows are taken in pairs (j, n_z-1-j), j = k/2,
+        // and the middle row (z = 0) alone at the end.
+        const int n_g = SYM ? (p.n_z + 1) / 2 : p.n_z;                        // templates fetched per segment
+        auto it_sel = [&](int k) { return SYM ? (k & 1) : 0; };
+        auto it_row = [&](int k) { return SYM ? ((k & 1) ? p.n_z - 1 - (k >> 1) : (k >> 1)) : k; };
+        auto it_last_use = [&](int k) { return SYM ? ((k & 1) || k == p.n_z - 1) : true; };
+        int g_next = 1; // elected thread: next template to fetch
 
         const int64_t col0 = seg * p.S - p.m + t;                             // column of y[t]
         float *__restrict__ out = p.power + bi * p.n_z * p.n_f + col0;        // row 0 of this batch item
+        float *const out0 = out;
         float2 *__restrict__ out_c = p.amp + bi * p.n_z * p.n_f + col0;
         int64_t bm_idx = (bi * p.n_z) * p.n_seg + seg;                         // OUT_BLOCKMAX: entry of row 0
         const bool interior = (seg + 1) * (int64_t)p.S <= p.n_f;
@@ -379,12 +408,15 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
 
         // a3 + first inverse pass of template z ("convolution in the Fourier domain"; "for every
         // matched filter"): v = X * G_z in layout P-1, butterflies of pass P-1
-        auto stage_a = [&]() {
+        auto stage_a = [&](int k) {
             float2 X[E];
-            ptx::tmem_ld16(tm_addr + TC::X_OFF, X);
-            if constexpr (E > 8) ptx::tmem_ld16(tm_addr + TC::X_OFF + 16, X + 8);
-            ptx::mbar_wait(&g_bar, gphase);
-            gphase ^= 1;
+            const uint32_t xa = tm_addr + (it_sel(k) ? XC_OFF : TC::X_OFF);
+            ptx::tmem_ld16(xa, X);
+            if constexpr (E > 8) ptx::tmem_ld16(xa + 16, X + 8);
+            if (!it_sel(k)) { // a new template: wait for its bulk copy
+                ptx::mbar_wait(&g_bar, gphase);
+                gphase ^= 1;
+            }
             ptx::tmem_wait_ld8(X);
             if constexpr (E > 8) ptx::tmem_wait_ld8(X + 8);
 #pragma unroll
@@ -395,22 +427,24 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
             }
             inv_stage_a<C>(v);
         };
-        // elected thread, every thread being past its reads of the stage: slot k < n_z is the template
-        // spectrum G_k, slot n_z the next work item's segment
-        auto fetch_slot = [&](int k) {
-            if (t == 0) {
-                if (k < p.n_z) {
+        // elected thread, after the barrier that follows stage A of iteration k (every thread is past its reads of
+        // the stage): if that was the last use of its template, fetch the next one, or after the last template the
+        // next work item's segment
+        auto after_stage_a = [&](int k) {
+            if (t == 0 && it_last_use(k)) {
+                if (g_next < n_g) {
                     ptx::mbar_expect_tx(&g_bar, G_BYTES);
-                    ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)k * G_BYTES, G_BYTES, &g_bar);
-                } else if (k == p.n_z && w_next < p.n_work && seg_bulk(w_next)) {
+                    ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)g_next * G_BYTES, G_BYTES, &g_bar);
+                } else if (g_next == n_g && w_next < p.n_work && seg_bulk(w_next)) {
                     fetch_segment(w_next);
                 }
+                ++g_next;
             }
         };
-        stage_a();
+        stage_a(0);
         __syncthreads(); // also: the forward transform's last reads of buf0 are done before the z loop writes it
         if (t == 0) s_work[slot ^ 1] = w_next;
-        fetch_slot(1);
+        after_stage_a(0);
 
         // The z loop is software pipelined: stage A of template z+1 (tensor-memory and shared-memory
         // reads, 1/3 of the arithmetic) sits between the exchange write of template z and its barrier, so
@@ -446,9 +480,9 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
             for (int z = 0; z < p.n_z; ++z) {
                 float2 *bufa = (C::P == 3 && (z & 1)) ? buf1 : buf0;
                 inv_stage_b<C>(v, bufa, A, tws, lane);
-                if (z + 1 < p.n_z) stage_a();
+                if (z + 1 < p.n_z) stage_a(z + 1);
                 __syncthreads();
-                fetch_slot(z + 2);
+                if (z + 1 < p.n_z) after_stage_a(z + 1);
                 if constexpr (OUT == OUT_BLOCKMAX) {
                     if (z > 0) finalize_max(z - 1);
                 }
@@ -456,6 +490,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
                 inv_stage_c<C>(u, bufa, buf1, A, tw0, tws);
                 // a5 + a6: trim, then power / amplitude / block maximum
                 if constexpr (OUT == OUT_POWER) {
+                    if constexpr (SYM) out = out0 + (int64_t)it_row(z) * p.n_f;
 #pragma unroll
                     for (int d = 0; d < E; ++d) {
                         if (MODE == 0 && d < D0_FAST) continue;
@@ -465,7 +500,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
                             else __stcs(out + d * NT, pw);
                         }
                     }
-                    out += p.n_f;
+                    if constexpr (!SYM) out += p.n_f;
                 } else if constexpr (OUT == OUT_AMP) {
 #pragma unroll
                     for (int d = 0; d < E; ++d) {

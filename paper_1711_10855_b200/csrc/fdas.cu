@@ -124,6 +124,9 @@ struct fdas_plan {
     int last_launches;
     int device;               // CUDA device the plan lives on (every call checks it)
     int grid_max[3];          // resident CTAs of the hot kernel per output mode (registers, smem, tensor memory)
+    int grid_max_sym;         // same for the +-z symmetric power kernel (0: this segment length has none)
+    bool sym_requested;       // fdas_plan_set_symmetry
+    bool sym_detected;        // the current bank satisfies h_{-z} = conj(h_{+z}) bit for bit
     unsigned int *d_work;     // [WORK_SLOTS][2] work counters of the persistent kernel, zero between launches
     unsigned int work_seq;    // launches so far: selects the counter pair
     // buffers of fdas_convolve_host
@@ -175,9 +178,9 @@ template <int L> size_t smem_bytes() { return 2 * sizeof(float2) * (size_t)InvCf
 // that run concurrently (several streams) use different pairs; a pair is re-armed by its own launch.
 constexpr unsigned WORK_SLOTS = 1024;
 
-template <int L, int OUT> cudaError_t launch_convolve(const ConvParams &cp, int grid_max, cudaStream_t st)
+template <int L, int OUT, bool SYM = false> cudaError_t launch_convolve(const ConvParams &cp, int grid_max, cudaStream_t st)
 {
-    auto kern = fdas_convolve_kernel<L, OUT>;
+    auto kern = fdas_convolve_kernel<L, OUT, SYM>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
     if (cp.n_work > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const unsigned grid = (unsigned)(cp.n_work < grid_max ? cp.n_work : grid_max);
@@ -189,9 +192,9 @@ template <int L, int OUT> cudaError_t launch_convolve(const ConvParams &cp, int 
 // memory and size the persistent grid = resident CTAs per SM x SMs.  Resident CTAs are counted here
 // from the kernel's registers and shared memory, the SM's thread / block limits and the tensor memory
 // (512 columns per SM); the occupancy API reports one CTA per SM for a kernel that allocates tensor memory.
-template <int L, int OUT> cudaError_t prepare_convolve(int device, int *grid_max)
+template <int L, int OUT, bool SYM = false> cudaError_t prepare_convolve(int device, int *grid_max)
 {
-    auto kern = fdas_convolve_kernel<L, OUT>;
+    auto kern = fdas_convolve_kernel<L, OUT, SYM>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
     constexpr int NT = Cfg<L>::NT;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -360,6 +363,9 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
         FDAS_DISPATCH_L(L, (e = prepare_convolve<LL, OUT_POWER>(p->device, &p->grid_max[OUT_POWER])));
         if (e == cudaSuccess) { FDAS_DISPATCH_L(L, (e = prepare_convolve<LL, OUT_AMP>(p->device, &p->grid_max[OUT_AMP]))); }
         if (e == cudaSuccess) { FDAS_DISPATCH_L(L, (e = prepare_convolve<LL, OUT_BLOCKMAX>(p->device, &p->grid_max[OUT_BLOCKMAX]))); }
+        // the symmetric kernel needs a free 32-column block of tensor memory: the three-pass, >= 128-thread plans
+        if (e == cudaSuccess && L == 2048) e = prepare_convolve<2048, OUT_POWER, true>(p->device, &p->grid_max_sym);
+        if (e == cudaSuccess && L == 4096) e = prepare_convolve<4096, OUT_POWER, true>(p->device, &p->grid_max_sym);
     }
     if (e != cudaSuccess) {
         fdas_status s = (e == cudaErrorMemoryAllocation) ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
@@ -401,7 +407,28 @@ fdas_status fdas_set_templates(fdas_plan *p, const float *h_templates)
     cudaFree(d_h);
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->has_templates = true;
+    // FDAS symmetry of the bank (SURVEY.md 8(c) note S): row n_z-1-i is the element-wise conjugate of row i, bit for
+    // bit (which makes the middle row, z = 0, real).  Anything else takes the general path.
+    bool sym = (p->n_z & 1) != 0;
+    for (int i = 0; sym && i <= p->n_z / 2; ++i) {
+        const float *a = h_templates + (size_t)2 * p->m * i, *b = h_templates + (size_t)2 * p->m * (p->n_z - 1 - i);
+        for (int j = 0; j < p->m; ++j)
+            if (a[2 * j] != b[2 * j] || a[2 * j + 1] != -b[2 * j + 1]) { sym = false; break; }
+    }
+    p->sym_detected = sym;
     return FDAS_OK;
+}
+
+fdas_status fdas_plan_set_symmetry(fdas_plan *p, int enable)
+{
+    if (!p) return FDAS_ERR_INVALID_ARG;
+    p->sym_requested = enable != 0;
+    return FDAS_OK;
+}
+
+int fdas_plan_symmetry_active(const fdas_plan *p)
+{
+    return p && p->sym_requested && p->sym_detected && p->grid_max_sym > 0;
 }
 
 // common part of the three entry points that enqueue the hot kernel
@@ -430,7 +457,14 @@ static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, f
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
     switch (out_mode) {
-    case OUT_POWER: FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_POWER>(cp, p->grid_max[OUT_POWER], st))); break;
+    case OUT_POWER:
+        if (p->sym_requested && p->sym_detected && p->grid_max_sym > 0) {
+            if (L == 2048) e = launch_convolve<2048, OUT_POWER, true>(cp, p->grid_max_sym, st);
+            else e = launch_convolve<4096, OUT_POWER, true>(cp, p->grid_max_sym, st);
+        } else {
+            FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_POWER>(cp, p->grid_max[OUT_POWER], st)));
+        }
+        break;
     case OUT_AMP: FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_AMP>(cp, p->grid_max[OUT_AMP], st))); break;
     case OUT_BLOCKMAX: FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_BLOCKMAX>(cp, p->grid_max[OUT_BLOCKMAX], st))); break;
     default: break;
