@@ -275,7 +275,6 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     if (t == 0) {
         ptx::mbar_init(&g_bar, 1);
         ptx::mbar_fence_init();
-        s_work[0] = atomicAdd(p.work, 1u);
     }
     if (warp == 0) ptx::tmem_alloc<TC::NCOLS>(&tmem_slot);
     ptx::tmem_fence_before_sync();
@@ -332,7 +331,9 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
         ptx::bulk_g2s(gs, src, G_BYTES, &g_bar);
     };
 
-    uint32_t w = s_work[0];
+    // Work items: the first is the CTA's own index, the others come from the counter (which therefore counts from
+    // gridDim.x).  A wave of CTAs that starts together would otherwise open with hundreds of atomics on one address.
+    uint32_t w = blockIdx.x;
     int slot = 0;
     if (t == 0 && w < p.n_work && seg_bulk(w)) fetch_segment(w);
 
@@ -340,7 +341,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
         const int64_t seg = w % p.n_seg;
         const int64_t bi = w / p.n_seg;
         uint32_t w_next = 0;
-        if (t == 0) w_next = atomicAdd(p.work, 1u); // consumed after the first barrier below
+        if (t == 0) w_next = (gridDim.x < p.n_work) ? gridDim.x + atomicAdd(p.work, 1u) : (uint32_t)p.n_work; // used after the next barriers
 
         // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
         float2 v[E];
@@ -435,15 +436,15 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
                 if (g_next < n_g) {
                     ptx::mbar_expect_tx(&g_bar, G_BYTES);
                     ptx::bulk_g2s(gs, reinterpret_cast<const unsigned char *>(p.gperm) + (size_t)g_next * G_BYTES, G_BYTES, &g_bar);
-                } else if (g_next == n_g && w_next < p.n_work && seg_bulk(w_next)) {
-                    fetch_segment(w_next);
+                } else if (g_next == n_g) { // first use of w_next: the atomic has had nearly the whole segment to return
+                    s_work[slot ^ 1] = w_next;
+                    if (w_next < p.n_work && seg_bulk(w_next)) fetch_segment(w_next);
                 }
                 ++g_next;
             }
         };
         stage_a(0);
         __syncthreads(); // also: the forward transform's last reads of buf0 are done before the z loop writes it
-        if (t == 0) s_work[slot ^ 1] = w_next;
         after_stage_a(0);
 
         // The z loop is software pipelined: stage A of template z+1 (tensor-memory and shared-memory
@@ -548,7 +549,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     ptx::tmem_fence_before_sync();
     __syncthreads();
     if (warp == 0) ptx::tmem_free<TC::NCOLS>(tmem_slot);
-    if (t == 0) { // the last CTA out re-arms the counters for the next launch
+    if (t == 0 && gridDim.x < p.n_work) { // the last CTA out re-arms the counters for the next launch
         __threadfence();
         if (atomicAdd(p.work + 1, 1u) == gridDim.x - 1) {
             p.work[0] = 0;

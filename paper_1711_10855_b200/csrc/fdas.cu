@@ -453,6 +453,7 @@ static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, f
     cp.m = p->m;
     cp.S = p->S;
     cp.bulk_ok = ((uintptr_t)d_spectrum & 15u) == 0;
+    if (getenv("FDAS_EXP_NOBULK")) cp.bulk_ok = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
@@ -671,6 +672,6 @@ int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b)
 }
 
 // The kernel generation is what profiles/traffic.json is keyed by: bump it with every change to the hot kernel.
-const char *fdas_version(void) { return "libfdas sm_100a k6"; }
+const char *fdas_version(void) { return "libfdas sm_100a k7"; }
 
 } // extern "C"

@@ -211,9 +211,13 @@ template <class C> struct InvCfg {
     static constexpr int Ra = C::R(P - 1), Rb = C::R(P - 2);
     static constexpr int Gs = Ra * Rb / E, NA = E / Rb, NB = E / Ra;
     static constexpr int Q = Ra * Rb;                       // points per group
-    static constexpr int PAD = Gs >= 16 ? 0 : 8;            // half-warp = several groups: offset them by 8 banks
-    // P == 3: one exchange, element (k_0, n_1, n_2) at k_0*STR0 + n_1*Ra + n_2
-    // P == 4: exchange A, element (k_0, k_1, n_2, n_3) at (k_0*R1 + k_1)*STRX + n_2*Ra + n_3,
+    // A half-warp spans 16/Gs groups.  Within a row of the exchange buffer the low index n_{P-1} = c*NA + j is stored
+    // at lo_pos = j*Gs + c, so that the Gs threads of a group write Gs CONSECUTIVE elements per store; padding every
+    // row by Gs elements then puts the groups of a half-warp on disjoint banks (64-bit accesses: 16 bank pairs).
+    static constexpr int PAD = Gs >= 16 ? 0 : Gs;
+    __host__ __device__ static constexpr int lo_pos(int n_lo) { return (n_lo % NA) * Gs + n_lo / NA; }
+    // P == 3: one exchange, element (k_0, n_1, n_2) at k_0*STR0 + n_1*Ra + lo_pos(n_2)
+    // P == 4: exchange A, element (k_0, k_1, n_2, n_3) at (k_0*R1 + k_1)*STRX + n_2*Ra + lo_pos(n_3),
     //         exchange B, element (k_0, n_1, n_2, n_3) at k_0*NT + n_1*Q + n_2*Ra + n_3
     static constexpr int STR0 = (P == 3) ? NT + PAD : NT;
     static constexpr int STRX = Q + PAD;
@@ -226,7 +230,7 @@ template <class C> struct InvCfg {
     __host__ __device__ static constexpr int shfl_src_reg(int r, int i, int j) { return i * Ra + NA * r + j; }
     __host__ __device__ static constexpr int shfl_dst_reg(int r, int i, int j) { return j * Rb + NB * r + NB - 1 - i; }
     // shared-memory offsets relative to InvAddr (complex elements)
-    __host__ __device__ static constexpr int wa_off(int j, int kap) { return ((Rb - kap) % Rb) * Ra + j; } // register j*Rb+kap
+    __host__ __device__ static constexpr int wa_off(int j, int kap) { return ((Rb - kap) % Rb) * Ra + j * Gs; } // register j*Rb+kap
     __host__ __device__ static constexpr int ra_off(int b, int k) { return P == 3 ? k * STR0 : (b * KK * C::R(1) + k) * STRX; }
     __host__ __device__ static constexpr int wb_off(int b, int n) { return KK * b * STR0 + n * Q; }         // P == 4 only
     __host__ __device__ static constexpr int rb_off(int k) { return k * STR0; }                             // P == 4 only
@@ -305,13 +309,15 @@ template <class C> __host__ __device__ __forceinline__ InvAddr<C> inv_addr(int t
 {
     using I = InvCfg<C>;
     InvAddr<C> A;
+    // thread t reads the element whose low index is t % Ra, stored at lo_pos(t % Ra) of its Ra-block
+    const int rd = t - (t % I::Ra) + I::lo_pos(t % I::Ra);
     if constexpr (C::P == 3) {
-        A.wa = (t / I::Gs) * I::STR0 + I::NA * (t % I::Gs);
-        A.ra = t;
+        A.wa = (t / I::Gs) * I::STR0 + (t % I::Gs);
+        A.ra = rd;
         A.wb = A.rb = 0;
     } else {
-        A.wa = (t / I::Gs) * I::STRX + I::NA * (t % I::Gs);
-        A.ra = (t / I::Q) * C::R(1) * I::STRX + (t % I::Q);
+        A.wa = (t / I::Gs) * I::STRX + (t % I::Gs);
+        A.ra = (t / I::Q) * C::R(1) * I::STRX + (rd % I::Q);
         A.wb = (t / I::Q) * I::STR0 + (t % I::Q);
         A.rb = t;
     }

@@ -173,3 +173,23 @@ def test_layout_query_rejects_bad_arguments():
     assert B.debug_layout(4096, B.LAYOUT_FREQ, 256, 0, 0) == -1    # thread out of range
     assert B.debug_layout(4096, 99, 0, 0, 0) == -1                 # unknown selector
     assert B.debug_layout(4096, B.LAYOUT_WRITE_B, 0, 0, 0) == -1   # three-pass plan has no second exchange
+
+
+@pytest.mark.parametrize("L", [512, 1024, 2048, 4096, 8192])
+def test_inverse_exchanges_are_bank_conflict_free(L):
+    """Every 64-bit shared-memory access of the hot loop's exchanges: the 16 threads of a half-warp fall on 16
+    distinct bank pairs (or on the same address).  Round 2 found the first-exchange writes of the NA = 2 plans
+    (L = 1024, 8192) two-way conflicted: 28 % of their shared-memory wavefronts (profiles/r2_all_configs.md)."""
+    g = lambda a: B.debug_layout(L, B.LAYOUT_GEOMETRY, 0, a)
+    P, E, NT, Ra, Rb, Gs, NA, NB, BUF, R0, R1 = [g(i) for i in range(11)]
+    accesses = [(B.LAYOUT_WRITE_A, NA, Rb), (B.LAYOUT_READ_A, E // (R0 if P == 3 else R1), R0 if P == 3 else R1)]
+    if P == 4:
+        accesses += [(B.LAYOUT_WRITE_B, E // R1, R1), (B.LAYOUT_READ_B, R0, 1)]
+    for what, n1, n2 in accesses:
+        for a in range(n1):
+            for b in range(n2):
+                addr = [B.debug_layout(L, what, t, a, b) for t in range(NT)]
+                assert min(addr) >= 0 and max(addr) < BUF
+                for h in range(0, NT, 16):
+                    distinct = set(addr[h:h + 16])
+                    assert len({x % 16 for x in distinct}) == len(distinct), (L, what, a, b, h)
