@@ -40,6 +40,8 @@ def lib():
         L.fdas_oracle_direct.restype = ctypes.c_int
         L.fdas_oracle_ols.argtypes = [dp, i64, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                       ctypes.c_int, ctypes.c_int, dp]
+        L.fdas_oracle_spectrum.argtypes = [dp, i64, i64, dp]
+        L.fdas_oracle_spectrum.restype = ctypes.c_int
         L.fdas_oracle_blockmax.argtypes = [dp, ctypes.c_int, i64, i64, ctypes.c_int, dp, ctypes.POINTER(ctypes.c_int64)]
         L.fdas_oracle_blockmax.restype = ctypes.c_int
         L.fdas_oracle_ols.restype = ctypes.c_int
@@ -162,3 +164,16 @@ def blockmax(power, blk, float32_decision=True):
     if rc != 0:
         raise ValueError("oracle blockmax: bad arguments")
     return mx, ar
+
+
+def spectrum(series, whiten_block=0):
+    """P:21 "the FFT output of the observation" (reading 18): eq.(3) of the real series, bins
+    0 .. n_t/2 - 1, whitened in blocks of `whiten_block` bins (0: not whitened).  complex128 [n_t/2]."""
+    x = np.ascontiguousarray(series, dtype=np.float64)
+    if x.ndim != 1:
+        raise ValueError("series must be one-dimensional")
+    out = np.empty(x.size // 2, dtype=np.complex128)
+    rc = lib().fdas_oracle_spectrum(_dp(x), x.size, int(whiten_block), _dp(out))
+    if rc != 0:
+        raise ValueError("oracle spectrum: bad arguments")
+    return out

@@ -19,6 +19,9 @@
  *                                         and its power |A'|^2 (the authority for parity)
  *   fdas_oracle_ols        P:31           the same plane by overlap-and-save in double, with
  *                                         fdas_oracle_fft (checked against fdas_oracle_direct)
+ *   fdas_oracle_spectrum   P:21           "the FFT output of the observation": eq.(3) of the real time series,
+ *                                         bins 0 .. n_t/2 - 1, each block of bins scaled to unit variance per
+ *                                         component (reading 18) -- the input of the correlation
  *   fdas_oracle_blockmax   P:21, P:50     the detection step that consumes the plane ("FDAS code";
  *                                         the paper leaves it to Dimoudi 2017, reading 17):
  *                                         per row and block of columns, the maximum power and the
@@ -389,5 +392,44 @@ int fdas_oracle_blockmax(const double *power, int n_rows, int64_t n_cols, int64_
             arg_out[(size_t)r * (size_t)n_blk + (size_t)b] = arg;
         }
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * The step before the correlation ("the FFT output of the observation"; SURVEY.md NEXT-3;
+ * DESIGN.md reading 18).  series: n_t real samples, n_t a power of two >= 4.
+ *   X_k = sum_n series[n] exp(-i 2 pi n k / n_t)                     eq.(3), k = 0 .. n_t/2 - 1
+ *   whitening: bins are cut into blocks of `blk` bins, block b = [b*blk, min((b+1)*blk, n_t/2));
+ *     m_b = mean over the block's bins of |X_k|^2, bin 0 (the DC term) counted as 0
+ *     A_k = X_k * sqrt(2 / m_b)   (each of re, im then has unit variance where the block is noise),
+ *     A_0 = 0, and A_k = 0 in a block with m_b = 0.   blk <= 0: no whitening, A_k = X_k.
+ * out: [n_t/2][2].  The transform is fdas_oracle_fft on the zero-imaginary complex sequence.
+ * ------------------------------------------------------------------------------------------ */
+int fdas_oracle_spectrum(const double *series, int64_t n_t, int64_t blk, double *out)
+{
+    if (!series || !out || n_t < 4 || (n_t & (n_t - 1))) return -1;
+    double *z = (double *)malloc(sizeof(double) * 2 * (size_t)n_t);
+    if (!z) return -1;
+    for (int64_t n = 0; n < n_t; ++n) { z[2 * n] = series[n]; z[2 * n + 1] = 0.0; }
+    if (fdas_oracle_fft(z, n_t, -1) != 0) { free(z); return -1; }
+    int64_t n_f = n_t / 2;
+    if (blk <= 0) {
+        memcpy(out, z, sizeof(double) * 2 * (size_t)n_f);
+        free(z);
+        return 0;
+    }
+    for (int64_t b0 = 0; b0 < n_f; b0 += blk) {
+        int64_t b1 = b0 + blk < n_f ? b0 + blk : n_f;
+        double sum = 0.0;
+        for (int64_t k = b0; k < b1; ++k)
+            if (k != 0) sum += z[2 * k] * z[2 * k] + z[2 * k + 1] * z[2 * k + 1];
+        double mean = sum / (double)(b1 - b0);
+        double scale = mean > 0.0 ? sqrt(2.0 / mean) : 0.0;
+        for (int64_t k = b0; k < b1; ++k) {
+            out[2 * k] = k == 0 ? 0.0 : z[2 * k] * scale;
+            out[2 * k + 1] = k == 0 ? 0.0 : z[2 * k + 1] * scale;
+        }
+    }
+    free(z);
     return 0;
 }
