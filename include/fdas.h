@@ -167,6 +167,25 @@ fdas_status fdas_fft_plan_destroy(fdas_fft_plan *plan);
 int fdas_fft_plan_elems_per_thread(const fdas_fft_plan *plan);
 int fdas_fft_plan_grid(const fdas_fft_plan *plan);   /* CTAs of one launch at most (grid-stride over the batch) */
 
+/*
+ * The step before the correlation ("the FFT output of the observation"; reading 18): the real
+ * time series of n_samples float32 samples -> its n_samples/2 lowest Fourier bins (eq.(3)), whitened.
+ *   n_samples     a power of two, 2^19 .. 2^27 (else FDAS_ERR_UNSUPPORTED); BASELINE.json config 3: 2^23
+ *   whiten_block  > 0: bins are cut into blocks of that many bins, block b = [b*blk, min((b+1)*blk, n/2)), and every
+ *                 block is scaled by sqrt(2 / mean |X_k|^2) (bin 0 counted as 0 and set to 0) so that re and im
+ *                 have unit variance where the block is noise; a block of zeros stays zero.  <= 0: not whitened.
+ *   d_series      DEVICE, float32 [n_samples], 8-byte aligned, read only
+ *   d_spectrum    DEVICE, complex64 [n_samples/2] -- what fdas_convolve takes as d_spectrum
+ * fdas_spectrum_exec enqueues six launches on the stream (three transposes, two batched segment FFTs, one
+ * separate-and-whiten pass) using two plan-owned scratch buffers of n_samples/2 complex64: one exec of a plan at a
+ * time.  Asynchronous; deterministic.
+ */
+typedef struct fdas_spectrum_plan fdas_spectrum_plan;
+fdas_status fdas_spectrum_plan_create(fdas_spectrum_plan **out, int64_t n_samples, int64_t whiten_block);
+fdas_status fdas_spectrum_exec(fdas_spectrum_plan *plan, const float *d_series, void *d_spectrum, void *cuda_stream);
+fdas_status fdas_spectrum_plan_destroy(fdas_spectrum_plan *plan);
+int64_t fdas_spectrum_plan_bins(const fdas_spectrum_plan *plan);  /* n_samples / 2 */
+
 /* Free the plan and everything it owns.  NULL is accepted. */
 fdas_status fdas_plan_destroy(fdas_plan *plan);
 

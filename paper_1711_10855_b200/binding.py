@@ -42,6 +42,10 @@ SYMBOLS = {
     "fdas_fft_plan_destroy": (_int, [_vp]),
     "fdas_fft_plan_elems_per_thread": (_int, [_vp]),
     "fdas_fft_plan_grid": (_int, [_vp]),
+    "fdas_spectrum_plan_create": (_int, [ctypes.POINTER(_vp), _i64, _i64]),
+    "fdas_spectrum_exec": (_int, [_vp, _vp, _vp, _vp]),
+    "fdas_spectrum_plan_destroy": (_int, [_vp]),
+    "fdas_spectrum_plan_bins": (_i64, [_vp]),
     "fdas_debug_fft": (_int, [_int, _i64, _vp, _vp, _int]),
     "fdas_debug_layout": (_i64, [_int, _int, _int, _int, _int]),
     "fdas_version": (ctypes.c_char_p, []),
@@ -206,6 +210,32 @@ class FftPlan:
     def destroy(self):
         if self._h:
             lib().fdas_fft_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class SpectrumPlan:
+    """fdas_spectrum_plan_create ... _destroy: real time series -> whitened complex spectrum."""
+
+    def __init__(self, n_samples, whiten_block=0):
+        self._h = _vp()
+        _check(lib().fdas_spectrum_plan_create(ctypes.byref(self._h), int(n_samples), int(whiten_block)),
+               "fdas_spectrum_plan_create")
+
+    @property
+    def bins(self): return lib().fdas_spectrum_plan_bins(self._h)
+
+    def exec(self, d_series, d_spectrum, stream=None):
+        _check(lib().fdas_spectrum_exec(self._h, _ptr(d_series), _ptr(d_spectrum), _stream(stream)), "fdas_spectrum_exec")
+
+    def destroy(self):
+        if self._h:
+            lib().fdas_spectrum_plan_destroy(self._h)
             self._h = _vp()
 
     def __del__(self):

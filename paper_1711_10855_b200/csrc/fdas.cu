@@ -19,6 +19,7 @@
 #include "fft_device.cuh"
 #include "convolve.cuh"
 #include "fft_batch.cuh"
+#include "spectrum.cuh"
 
 namespace fdas {
 
@@ -332,6 +333,16 @@ template <class C> static cudaError_t fft_batch_launch(const fdas_fft_plan *p, i
     else if ((N) == 4096 && (E) == 16) { using CC = Cfg<4096>; EXPR; }             \
     else if ((N) == 8192 && (E) == 16) { using CC = Cfg<8192>; EXPR; }
 
+// -------------------------------------------------------------------------------------------
+// spectrum of the observation (NEXT-3): real series -> whitened complex spectrum
+// -------------------------------------------------------------------------------------------
+struct fdas_spectrum_plan {
+    int64_t n_t, N, blk;
+    int N1, N2, device;
+    fdas_fft_plan *f1, *f2;   // batched transforms of length N1 and N2
+    float2 *d_a, *d_b;        // scratch, N complex each
+};
+
 extern "C" {
 
 fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step, int template_width, int segment_len)
@@ -634,6 +645,76 @@ fdas_status fdas_fft_plan_destroy(fdas_fft_plan *p)
 
 int fdas_fft_plan_elems_per_thread(const fdas_fft_plan *p) { return p ? p->e : 0; }
 int fdas_fft_plan_grid(const fdas_fft_plan *p) { return p ? p->grid_max : 0; }
+
+fdas_status fdas_spectrum_plan_destroy(fdas_spectrum_plan *p)
+{
+    if (!p) return FDAS_OK;
+    fdas_fft_plan_destroy(p->f1);
+    fdas_fft_plan_destroy(p->f2);
+    if (p->d_a) cudaFree(p->d_a);
+    if (p->d_b) cudaFree(p->d_b);
+    (void)cudaGetLastError();
+    free(p);
+    return FDAS_OK;
+}
+
+fdas_status fdas_spectrum_plan_create(fdas_spectrum_plan **out, int64_t n_samples, int64_t whiten_block)
+{
+    if (!out || n_samples < 4 || (n_samples & (n_samples - 1))) return FDAS_ERR_INVALID_ARG;
+    int k = 0;
+    while (((int64_t)1 << k) < n_samples / 2) ++k;          // N = 2^k complex points
+    if (k < 18 || k > 26) return FDAS_ERR_UNSUPPORTED;       // N = N1 N2 with both factors in 512 .. 8192
+    fdas_spectrum_plan *p = (fdas_spectrum_plan *)calloc(1, sizeof(fdas_spectrum_plan));
+    if (!p) return FDAS_ERR_ALLOC;
+    p->n_t = n_samples;
+    p->N = n_samples / 2;
+    p->blk = whiten_block > 0 ? whiten_block : 0;
+    p->N1 = 1 << ((k + 1) / 2);
+    p->N2 = 1 << (k / 2);
+    fdas_status s = fdas_fft_plan_create(&p->f1, p->N1, 0);
+    if (s == FDAS_OK) s = fdas_fft_plan_create(&p->f2, p->N2, 0);
+    cudaError_t e = cudaSuccess;
+    if (s == FDAS_OK) e = cudaGetDevice(&p->device);
+    if (s == FDAS_OK && e == cudaSuccess) e = cudaMalloc((void **)&p->d_a, sizeof(float2) * (size_t)p->N);
+    if (s == FDAS_OK && e == cudaSuccess) e = cudaMalloc((void **)&p->d_b, sizeof(float2) * (size_t)p->N);
+    if (s != FDAS_OK || e != cudaSuccess) {
+        (void)cudaGetLastError();
+        fdas_spectrum_plan_destroy(p);
+        return s != FDAS_OK ? s : (e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA);
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+fdas_status fdas_spectrum_exec(fdas_spectrum_plan *p, const float *d_series, void *d_spectrum, void *cuda_stream)
+{
+    if (!p || !d_series || !d_spectrum) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_series & 7u) || ((uintptr_t)d_spectrum & 7u)) return FDAS_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return FDAS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const float2 *z = (const float2 *)d_series;  // z[n] = x[2n] + i x[2n+1], viewed as [N1][N2]
+    const dim3 thr(32, 8);
+    // z [N1][N2] -> a [N2][N1];  N2 transforms of length N1: a -> b [n2][k1]
+    fdas_transpose_kernel<false><<<dim3(p->N2 / 32, p->N1 / 32), thr, 0, st>>>(z, p->d_a, p->N1, p->N2, p->N);
+    fdas_status s = fdas_fft_exec(p->f1, p->N2, p->d_a, p->d_b, 0, cuda_stream);
+    if (s != FDAS_OK) return s;
+    // b [N2][N1] times w_N^{n2 k1} -> a [k1][n2];  N1 transforms of length N2: a -> b [k1][k2] = Z[k1 + N1 k2]
+    fdas_transpose_kernel<true><<<dim3(p->N1 / 32, p->N2 / 32), thr, 0, st>>>(p->d_b, p->d_a, p->N2, p->N1, p->N);
+    s = fdas_fft_exec(p->f2, p->N1, p->d_a, p->d_b, 0, cuda_stream);
+    if (s != FDAS_OK) return s;
+    // b [N1][N2] -> a [k2][k1]: Z in natural order;  then separate the two real transforms and whiten
+    fdas_transpose_kernel<false><<<dim3(p->N2 / 32, p->N1 / 32), thr, 0, st>>>(p->d_b, p->d_a, p->N1, p->N2, p->N);
+    const long long width = p->blk > 0 ? p->blk : 4096;
+    const long long n_cta = (p->N + width - 1) / width;
+    if (n_cta > 0x7fffffffLL) return FDAS_ERR_INVALID_ARG;
+    fdas_rfft_whiten_kernel<<<(unsigned)n_cta, 256, 0, st>>>(p->d_a, (float2 *)d_spectrum, p->N, p->blk);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    return FDAS_OK;
+}
+
+int64_t fdas_spectrum_plan_bins(const fdas_spectrum_plan *p) { return p ? p->N : 0; }
 
 const char *fdas_status_string(fdas_status s)
 {
