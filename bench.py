@@ -62,7 +62,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the plane the oracle is timed on (0 = auto)")
-    ap.add_argument("--mode", default="convolve", choices=["convolve", "fft"],
+    ap.add_argument("--mode", default="convolve", choices=["convolve", "fft", "peak"],
                     help="convolve: the FDAS hot path (BASELINE.json metric); fft: the stand-alone FFT protocol of Table 1")
     ap.add_argument("--fft-n", type=int, default=1024)
     ap.add_argument("--no-detect", action="store_true", help="skip the fused block-maximum (detection) timings")
@@ -462,6 +462,36 @@ def run_fft(args):
     return 0
 
 
+def run_peak(args):
+    """--mode peak: the FP32 FMA rate of this GPU on register-only chains (fdas_debug_alu_peak) next to the nominal
+    figure the "alu" roofline uses, with the clocks seen meanwhile."""
+    import torch
+    from paper_1711_10855_b200 import binding
+    binding.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    pk = peaks()
+    nominal = N_SM * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.25)
+    t0 = time.time()
+    rows = []
+    for _ in range(max(1, min(args.steps, 10))):
+        for packed in (False, True):
+            tf, ms = binding.debug_alu_peak(packed)
+            rows.append({"form": "FFMA2 (packed)" if packed else "FFMA (scalar)", "tflops": tf, "ms": ms,
+                         "frac_of_nominal": tf / nominal, "lanes_per_clk_per_sm": tf * 1e12 / 2 / N_SM / (pk["sm_max_mhz"] * 1e6)})
+    clocks = sampler.stop(t0, time.time())
+    best = max(r["tflops"] for r in rows)
+    print(json.dumps({"metric": "fp32_fma_peak_tflops", "value": best, "unit": "TFLOP/s", "n_gpus": 1, "nominal_tflops": nominal,
+                      "nominal_def": f"{N_SM} SMs x {FP32_LANES_PER_SM} lanes x 2 x {pk['sm_max_mhz']:.0f} MHz",
+                      "best_scalar": max(r["tflops"] for r in rows if "scalar" in r["form"]),
+                      "best_packed": max(r["tflops"] for r in rows if "packed" in r["form"]),
+                      "runs": rows, "clocks": clocks, "higher_is_better": True, "data": "synthetic"}))
+    return 0
+
+
 def run_dry(args):
     """--dry-run: everything of the N-rank path that needs no GPU (gloo): rendezvous, per-rank seeded
     workload shape, MAX-over-ranks of a per-rank time, whole-job value.  Prints the JSON line with
@@ -510,6 +540,8 @@ def main():
         return run_dry(args)
     if args.mode == "fft":
         return run_fft(args)
+    if args.mode == "peak":
+        return run_peak(args)
     return run_ours(args)
 
 

@@ -238,6 +238,13 @@ enum {
 };
 int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b);
 
+/*
+ * Measurement support (bench.py --mode peak): the FP32 FMA rate this GPU reaches on register-only chains of
+ * dependent FMAs, scalar (packed = 0) or packed FFMA2 (packed = 1), in TFLOP/s by CUDA events.  It is what the
+ * nominal "alu" peak of the roofline (SMs x 128 lanes x 2 x max clock) is checked against.  Synchronous.
+ */
+fdas_status fdas_debug_alu_peak(int packed, double *tflops_out, double *ms_out);
+
 /* Library build info: e.g. "libfdas sm_100a <date>".  Never NULL. */
 const char *fdas_version(void);
 

@@ -48,6 +48,7 @@ SYMBOLS = {
     "fdas_spectrum_plan_bins": (_i64, [_vp]),
     "fdas_debug_fft": (_int, [_int, _i64, _vp, _vp, _int]),
     "fdas_debug_layout": (_i64, [_int, _int, _int, _int, _int]),
+    "fdas_debug_alu_peak": (_int, [_int, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
     "fdas_version": (ctypes.c_char_p, []),
 }
 
@@ -258,3 +259,10 @@ def debug_fft(segment_len, n_seg, d_in, d_out, inverse=False):
 def debug_layout(segment_len, what, t=0, a=0, b=0) -> int:
     """Host evaluation of the kernels' index maps (no GPU needed); -1 = out of range."""
     return int(lib().fdas_debug_layout(int(segment_len), int(what), int(t), int(a), int(b)))
+
+
+def debug_alu_peak(packed=False):
+    """(TFLOP/s, ms) of the register-only FMA chains of fdas_debug_alu_peak."""
+    tf, ms = ctypes.c_double(), ctypes.c_double()
+    _check(lib().fdas_debug_alu_peak(int(bool(packed)), ctypes.byref(tf), ctypes.byref(ms)), "fdas_debug_alu_peak")
+    return tf.value, ms.value

@@ -296,6 +296,33 @@ template <int L> static int64_t layout_query(int what, int t, int a, int b)
 }
 
 // -------------------------------------------------------------------------------------------
+// FP32 peak probe (measurement support, not on any path): every thread runs independent chains of dependent
+// FFMA (scalar, or packed FFMA2), ITER x CHAINS per thread; bench.py --mode peak divides the flops by the
+// event time.  This is what the "alu" roofline's 148 x 128 lanes x 2 x clock is checked against.
+// -------------------------------------------------------------------------------------------
+namespace fdas {
+template <bool PACKED> __global__ void __launch_bounds__(512) fdas_alu_peak_kernel(float *out, float c, int iters)
+{
+    constexpr int CH = 16;
+    float2 a[CH];
+#pragma unroll
+    for (int i = 0; i < CH; ++i) a[i] = make_float2(threadIdx.x + i, i);
+    const float2 cc = make_float2(c, c);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < CH; ++i) {
+            if (PACKED) a[i] = __ffma2_rn(a[(i + 1) % CH], cc, a[i]);
+            else { a[i].x = fmaf(a[(i + 1) % CH].x, c, a[i].x); a[i].y = fmaf(a[(i + 1) % CH].y, c, a[i].y); }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < CH; ++i) s += a[i].x + a[i].y;
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+} // namespace fdas
+
+// -------------------------------------------------------------------------------------------
 // stand-alone batched FFT (NEXT-4; Table 1)
 // -------------------------------------------------------------------------------------------
 struct fdas_fft_plan {
@@ -742,6 +769,39 @@ fdas_status fdas_debug_fft(int segment_len, int64_t n_seg, const void *d_in, voi
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (d_tw) cudaFree(d_tw);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    return FDAS_OK;
+}
+
+fdas_status fdas_debug_alu_peak(int packed, double *tflops_out, double *ms_out)
+{
+    if (!tflops_out) return FDAS_ERR_INVALID_ARG;
+    int dev = 0, n_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    float *d_out = nullptr;
+    const int blocks = 4 * (n_sm > 0 ? n_sm : 1), iters = 4000;
+    if (e == cudaSuccess) e = cudaMalloc((void **)&d_out, sizeof(float) * 512 * (size_t)blocks);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) {
+        for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) { // the last of three launches is the timed one
+            cudaEventRecord(e0);
+            if (packed) fdas_alu_peak_kernel<true><<<blocks, 512>>>(d_out, 1.0001f, iters);
+            else fdas_alu_peak_kernel<false><<<blocks, 512>>>(d_out, 1.0001f, iters);
+            cudaEventRecord(e1);
+            e = cudaEventSynchronize(e1);
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        }
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (d_out) cudaFree(d_out);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    const double flops = 2.0 * 2.0 * 16.0 * (double)iters * 512.0 * (double)blocks; // 2 flops x 2 lanes x chains x iters x threads
+    *tflops_out = flops / ((double)ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = ms;
     return FDAS_OK;
 }
 
