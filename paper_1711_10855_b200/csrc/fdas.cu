@@ -223,6 +223,7 @@ template <int L, int OUT, bool SYM = false> cudaError_t prepare_convolve(int dev
     if (per_sm > 512 / TmemCfg<Cfg<L>>::NCOLS) per_sm = 512 / TmemCfg<Cfg<L>>::NCOLS;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *grid_max = per_sm * n_sm;
+    // experiment knob (profiles/r2_c3_k6.md, r2_all_configs.md: grid-size sweeps); not part of the interface
     if (const char *g = getenv("FDAS_EXP_GRID")) *grid_max = atoi(g);
     return cudaSuccess;
 }
@@ -491,7 +492,7 @@ static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, f
     cp.m = p->m;
     cp.S = p->S;
     cp.bulk_ok = ((uintptr_t)d_spectrum & 15u) == 0;
-    if (getenv("FDAS_EXP_NOBULK")) cp.bulk_ok = 0;
+    if (getenv("FDAS_EXP_NOBULK")) cp.bulk_ok = 0; // experiment knob: guarded loads for every segment
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
