@@ -1,7 +1,8 @@
 // convolve.cuh -- the FDAS hot kernel (steps a1..a6 of DESIGN.md) for sm_100a.
 //
-// One CTA owns one (batch item, segment) and loops over all n_z templates ("for every matched
-// filter": multiply, inverse FFT, store).  Where the loop-invariant data live:
+// A persistent wave of CTAs; each takes (batch item, segment) work items one after the other and loops over
+// all n_z templates of the item ("for every matched filter": multiply, inverse FFT, store).  Where the
+// loop-invariant data live:
 //   * the forward-transformed segment X and the per-thread inverse twiddles of the passes after the
 //     first live in TENSOR MEMORY (tcgen05.st once per segment, tcgen05.ld per z): TMEM is a 256 KB
 //     per-SM array with its own data path (measured 930 B/clk/SM), so these reads cost neither
@@ -13,7 +14,9 @@
 // The inverse transform (fft_device.cuh, "Inverse transform of the hot loop") exchanges data once
 // by warp shuffles and once (L = 8192: twice) through shared memory; one barrier per exchange.
 // The z loop is software pipelined: stage A of template z+1 runs before the barrier of template z.
-// Measured cost model, ablations and the experiments that did not help: profiles/r1_c3_v4.md.
+// The same kernel has three outputs (power plane, complex plane, fused block maxima) and a variant for
+// symmetric template banks.  Measured cost model, ablations and the experiments that did not help:
+// profiles/r1_c3_v4.md, profiles/r2_c3_k6.md, profiles/r2_c3_k7.md.
 #pragma once
 #include <type_traits>
 

@@ -2,10 +2,11 @@
 //
 // arXiv:1711.10855 (P:NN = PAPER.md line NN): eq.(2) P:23 evaluated by overlap-and-save with
 // an on-chip FFT (eq.(3)) that is called once forward per segment and once inverse
-// per matched filter ("called for every matched filter").  One CTA owns one segment: the
+// per matched filter ("called for every matched filter").  A CTA owns one segment at a time: the
 // forward-transformed segment stays ON CHIP (tensor memory) across all n_z templates, so the spectrum
 // is read from HBM once per segment and the only HBM stream of the z loop is the coalesced power-plane
-// write.  The kernels are in convolve.cuh / fft_device.cuh; this file holds the C ABI.
+// write.  The kernels are in convolve.cuh / fft_device.cuh (hot path), fft_batch.cuh (stand-alone FFT) and
+// spectrum.cuh (the real-FFT + whitening step before the correlation); this file holds the C ABI.
 //
 // Built for sm_100a only.  No cuFFT, no CPU fallback.
 #include <cuda_runtime.h>
