@@ -62,7 +62,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the plane the oracle is timed on (0 = auto)")
-    ap.add_argument("--mode", default="convolve", choices=["convolve", "fft", "peak"],
+    ap.add_argument("--mode", default="convolve", choices=["convolve", "fft", "peak", "general"],
                     help="convolve: the FDAS hot path (BASELINE.json metric); fft: the stand-alone FFT protocol of Table 1")
     ap.add_argument("--fft-n", type=int, default=1024)
     ap.add_argument("--no-detect", action="store_true", help="skip the fused block-maximum (detection) timings")
@@ -462,6 +462,53 @@ def run_fft(args):
     return 0
 
 
+def run_general(args):
+    """--mode general: the shape of the paper's Table 2 on the complex-output convolution
+    (fdas_convolve_complex): filter lengths 64, 128, 256, 384, 512 on segments of 2048 points, the largest the paper's
+    FFT supports.  The table's entries are speed-ups over the authors' cuFFT-based and older codes on
+    P100 / TITAN X, none of which exists here: times and throughputs only."""
+    import torch
+    from paper_1711_10855_b200 import binding, workload
+    binding.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    n_f, z_max, z_step, L = 1 << 21, 84, 2, 2048           # the C4 sweep's spectrum and template grid
+    spec = [torch.from_numpy(workload.noise_spectrum(n_f, workload.SEED_BASE + 4000 + i, 1)).cuda() for i in range(8)]
+    n_z = 2 * z_max // z_step + 1
+    d_amp = torch.empty((1, n_z, n_f), dtype=torch.complex64, device="cuda")      # 1.43 GB >> L2
+    stream = torch.cuda.Stream()
+    pk = peaks()
+    fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    rows, launches = [], 0
+    for m in (64, 128, 256, 384, 512):
+        plan = binding.Plan(n_f, z_max, z_step, m, L)
+        plan.set_templates(workload.templates(z_max, z_step, m).astype(np.complex64))
+        for i in range(max(3, args.warmup)):
+            plan.convolve_complex(spec[i % 8], d_amp, stream=stream)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(args.steps):
+            plan.convolve_complex(spec[i % 8], d_amp, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        launches += args.steps
+        n_seg = plan.n_seg
+        flops = n_seg * (1 + n_z) * 5.0 * L * np.log2(L)
+        byt = 8 * n_z * n_f + 8 * n_seg * L + 8 * n_z * L
+        rows.append({"filter_length": m, "segments": int(n_seg), "ms": ms, "points_per_s": n_z * n_f / (ms * 1e-3),
+                     "alu_frac": flops / (ms * 1e-3) / 1e12 / fp32_peak, "hbm_frac": byt / (ms * 1e-3) / 1e9 / pk["hbm_gbs"]})
+        plan.destroy()
+    print(json.dumps({"metric": "general_convolution_points_per_s", "value": rows[-1]["points_per_s"], "unit": "points/s",
+                      "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "higher_is_better": True,
+                      "dtype": "f32", "data": "synthetic", "gpu_launches": launches,
+                      "config": {"workload": f"complex64 output, N_f={n_f}, {n_z} filters, L={L}, filter lengths 64..512 (Table 2, P:62-70)"},
+                      "rows": rows,
+                      "paper_context": "Table 2 lists speed-ups over cuFFT-based convolution (2.45-3.89 on P100): comparison codes absent, not reproducible"}))
+    return 0
+
+
 def run_peak(args):
     """--mode peak: the FP32 FMA rate of this GPU on register-only chains (fdas_debug_alu_peak) next to the nominal
     figure the "alu" roofline uses, with the clocks seen meanwhile."""
@@ -542,6 +589,8 @@ def main():
         return run_fft(args)
     if args.mode == "peak":
         return run_peak(args)
+    if args.mode == "general":
+        return run_general(args)
     return run_ours(args)
 
 
