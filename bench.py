@@ -360,7 +360,7 @@ def run_ours(args):
             "unit": "TFLOP/s" if alu_binds else "GB/s",
             "frac": (ach_tf / fp32_peak) if alu_binds else (ach_gb / pk["hbm_gbs"]),
             "traffic": traffic[0], "traffic_source": traffic[1],
-            "kernel": f"fdas::fdas_convolve_kernel<{wl.seg_len}>", "kernel_ms": kern_ms, "kernel_ms_min": float(np.min(per_launch_ms)),
+            "kernel": f"fdas::fdas_convolve_kernel<{wl.seg_len}, OUT_POWER, false>", "kernel_ms": kern_ms, "kernel_ms_min": float(np.min(per_launch_ms)),
             "flops_per_launch": flops_alg, "bytes_per_launch": bytes_alg,
             "alu": {"achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach_tf / fp32_peak,
                     "peak_def": f"{N_SM} SMs x {FP32_LANES_PER_SM} lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (nominal; flops = 5 L log2 L per transform)"},

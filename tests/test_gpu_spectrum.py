@@ -103,3 +103,18 @@ def test_spectrum_arguments():
     with pytest.raises(binding.FdasError) as ei:
         binding.SpectrumPlan((1 << 20) + 2)
     assert ei.value.status == binding.FDAS_ERR_INVALID_ARG
+
+
+def test_spectrum_is_deterministic():
+    import torch
+    from paper_1711_10855_b200 import binding
+    n_t = 1 << 21
+    x = torch.from_numpy(_series(n_t, 3, red=1.0)).cuda()
+    plan = binding.SpectrumPlan(n_t, 1500)
+    outs = [torch.empty(n_t // 2, dtype=torch.complex64, device="cuda") for _ in range(3)]
+    for o in outs:
+        plan.exec(x, o)
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0].view(torch.float32), outs[1].view(torch.float32))
+    assert torch.equal(outs[0].view(torch.float32), outs[2].view(torch.float32))
+    plan.destroy()
