@@ -97,9 +97,11 @@ int fdas_plan_symmetry_active(const fdas_plan *plan);
 /*
  * Enqueue the hot path on cuda_stream: for every batch item, segment and trial z -- segment load,
  * forward FFT (once per segment), pointwise multiply, inverse FFT, trim, |.|^2, power-plane write.
- *   d_spectrum    DEVICE, complex64 [n_batch][n_f], read only, 8-byte aligned
+ *   d_spectrum    DEVICE, complex64 [n_batch][n_f], read only, 8-byte aligned (16-byte alignment lets interior
+ *                 segments be staged by the bulk-copy engine; otherwise they are loaded with plain loads)
  *   d_power       DEVICE, float32 [n_batch][n_z][n_f], written completely, 4-byte aligned (128-byte
- *                 alignment and n_f % 32 == 0 give fully coalesced line writes)
+ *                 alignment and n_f % 32 == 0 give fully coalesced line writes; rows 32 bytes off the line
+ *                 grid cost 0.5 %, rows 4 bytes off 3.3 % on config 3: profiles/r2_c3_k7.md)
  *   cuda_stream   a cudaStream_t passed as void* (NULL = the legacy default stream)
  * Asynchronous: only launches; never synchronises, allocates or copies.  The buffers must stay
  * valid until the stream has run the work.  Output is bitwise reproducible (the kernel hands out
