@@ -141,7 +141,9 @@ fdas_status fdas_convolve_complex(fdas_plan *plan, const void *d_spectrum, void 
  *   d_max, d_arg  DEVICE, [n_batch][n_z][n_blk], 4-byte aligned, written completely
  * Comparisons are made on the float32 powers; equal powers resolve to the lowest column.  Deterministic.
  * Otherwise as fdas_convolve (asynchronous, same errors).  fdas_detect_blockmax_host is the HOST-pointer
- * convenience (spectrum in, the two small arrays out; synchronises the stream), like fdas_convolve_host.
+ * convenience (spectrum in, the two small arrays out; synchronises the stream), like fdas_convolve_host; when the
+ * call is several waves of work it uploads the spectrum in up to 8 pieces on a plan-owned copy stream and launches
+ * each piece's segments as it arrives, so that most of the host-to-device copy hides behind the kernel.
  */
 fdas_status fdas_detect_blockmax(fdas_plan *plan, const void *d_spectrum, float *d_max, int32_t *d_arg, void *cuda_stream);
 fdas_status fdas_detect_blockmax_host(fdas_plan *plan, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream);

@@ -226,7 +226,8 @@ struct ConvParams {
     unsigned int *__restrict__ work;     // [2] : next work item, CTAs finished (both 0 between launches)
     int64_t n_f;
     int64_t n_seg;
-    int64_t n_work;                      // n_batch * n_seg
+    int64_t n_work;                      // one past the last work item of this launch (n_batch * n_seg for a whole call)
+    int64_t w_begin;                     // first work item of this launch (0 for a whole call)
     int n_z;
     int m;
     int S;
@@ -336,7 +337,8 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
 
     // Work items: the first is the CTA's own index, the others come from the counter (which therefore counts from
     // gridDim.x).  A wave of CTAs that starts together would otherwise open with hundreds of atomics on one address.
-    uint32_t w = blockIdx.x;
+    const uint32_t n_mine = (uint32_t)(p.n_work - p.w_begin); // items of this launch
+    uint32_t w = (uint32_t)p.w_begin + blockIdx.x;
     int slot = 0;
     if (t == 0 && w < p.n_work && seg_bulk(w)) fetch_segment(w);
 
@@ -344,7 +346,8 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
         const int64_t seg = w % p.n_seg;
         const int64_t bi = w / p.n_seg;
         uint32_t w_next = 0;
-        if (t == 0) w_next = (gridDim.x < p.n_work) ? gridDim.x + atomicAdd(p.work, 1u) : (uint32_t)p.n_work; // used after the next barriers
+        if (t == 0) // used after the next barriers
+            w_next = (gridDim.x < n_mine) ? (uint32_t)p.w_begin + gridDim.x + atomicAdd(p.work, 1u) : (uint32_t)p.n_work;
 
         // a1: segment load, x[i] = A[seg*S - m/2 + i], zero outside [0, n_f)  (reading 6)
         float2 v[E];
@@ -552,7 +555,7 @@ __global__ void __launch_bounds__(Cfg<L>::NT, TmemCfg<Cfg<L>>::MINB) fdas_convol
     ptx::tmem_fence_before_sync();
     __syncthreads();
     if (warp == 0) ptx::tmem_free<TC::NCOLS>(tmem_slot);
-    if (t == 0 && gridDim.x < p.n_work) { // the last CTA out re-arms the counters for the next launch
+    if (t == 0 && gridDim.x < n_mine) { // the last CTA out re-arms the counters for the next launch
         __threadfence();
         if (atomicAdd(p.work + 1, 1u) == gridDim.x - 1) {
             p.work[0] = 0;

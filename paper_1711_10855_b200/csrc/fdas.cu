@@ -114,6 +114,8 @@ __global__ void __launch_bounds__(Cfg<L>::NT) fdas_debug_fft_kernel(const float2
 // =============================================================================================
 using namespace fdas;
 
+constexpr int HOST_CHUNKS = 8; // at most this many pieces of the host-to-device copy in fdas_detect_blockmax_host
+
 struct fdas_plan {
     int64_t n_f;
     int z_max, z_step, n_z, m, L, S;
@@ -136,6 +138,8 @@ struct fdas_plan {
     float *d_host_power;
     void *d_host_det;
     size_t host_spec_bytes, host_power_bytes, host_det_bytes;
+    cudaStream_t copy_stream;                 // fdas_detect_blockmax_host: chunked upload overlapping the kernel
+    cudaEvent_t copy_event[HOST_CHUNKS + 1];
 };
 
 namespace {
@@ -185,7 +189,9 @@ template <int L, int OUT, bool SYM = false> cudaError_t launch_convolve(const Co
     auto kern = fdas_convolve_kernel<L, OUT, SYM>;
     constexpr size_t smem = conv_smem_bytes<Cfg<L>>();
     if (cp.n_work > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    const unsigned grid = (unsigned)(cp.n_work < grid_max ? cp.n_work : grid_max);
+    const int64_t n_mine = cp.n_work - cp.w_begin;
+    if (n_mine <= 0) return cudaSuccess;
+    const unsigned grid = (unsigned)(n_mine < grid_max ? n_mine : grid_max);
     kern<<<grid, Cfg<L>::NT, smem, st>>>(cp);
     return cudaGetLastError();
 }
@@ -473,7 +479,7 @@ int fdas_plan_symmetry_active(const fdas_plan *p)
 
 // common part of the three entry points that enqueue the hot kernel
 static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, float *d_power, float2 *d_amp,
-                           float *d_max, int *d_arg, void *cuda_stream)
+                           float *d_max, int *d_arg, void *cuda_stream, int64_t w_begin = 0, int64_t w_end = -1)
 {
     if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
@@ -488,7 +494,8 @@ static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, f
     cp.work = p->d_work + 2 * (p->work_seq++ % WORK_SLOTS);
     cp.n_f = p->n_f;
     cp.n_seg = p->n_seg;
-    cp.n_work = p->n_seg * (int64_t)p->n_batch;
+    cp.n_work = w_end >= 0 ? w_end : p->n_seg * (int64_t)p->n_batch;
+    cp.w_begin = w_begin;
     cp.n_z = p->n_z;
     cp.m = p->m;
     cp.S = p->S;
@@ -582,10 +589,54 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, floa
     float *d_max = (float *)p->d_host_det;
     int32_t *d_arg = (int32_t *)p->d_host_det + nb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
+    // The spectrum goes up in HOST_CHUNKS pieces on a plan-owned copy stream and every piece's segments are launched
+    // as soon as it has arrived, so that all but the first piece of the host-to-device copy hides behind the kernel.
+    // The pieces are ranges of work items = (batch item, segment) in order, i.e. contiguous ranges of the input.
+    const int64_t n_work = p->n_seg * (int64_t)p->n_batch;
+    // Every piece is about one full wave of the persistent grid or more: smaller launches would leave SMs idle.
+    // A call that is a single wave anyway goes the plain way: copy, launch and read back on the caller's stream.
+    const int64_t waves = (n_work + p->grid_max[OUT_BLOCKMAX] - 1) / p->grid_max[OUT_BLOCKMAX];
+    const int n_chunks = (int)(waves > HOST_CHUNKS ? HOST_CHUNKS : waves);
+    if (n_chunks <= 1) {
+        e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        fdas_status s1 = fdas_detect_blockmax(p, p->d_host_spec, d_max, d_arg, cuda_stream);
+        if (s1 != FDAS_OK) return s1;
+        e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        return FDAS_OK;
+    }
+    if (!p->copy_stream) {
+        e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
+        for (int i = 0; e == cudaSuccess && i <= HOST_CHUNKS; ++i) e = cudaEventCreateWithFlags(&p->copy_event[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+    }
+    e = cudaEventRecord(p->copy_event[HOST_CHUNKS], st);                  // the copies start after the caller's earlier work
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, p->copy_event[HOST_CHUNKS], 0);
     if (e != cudaSuccess) return cuda_fail(p, e);
-    fdas_status s = fdas_detect_blockmax(p, p->d_host_spec, d_max, d_arg, cuda_stream);
-    if (s != FDAS_OK) return s;
+    size_t copied = 0; // complex elements of the flattened [n_batch][n_f] spectrum on the device so far
+    for (int c = 0; c < n_chunks; ++c) {
+        const int64_t w0 = n_work * c / n_chunks, w1 = n_work * (c + 1) / n_chunks;
+        // the last item of the piece is (bi, seg) = ((w1-1) / n_seg, (w1-1) % n_seg): it reads bins up to seg*S - m/2 + L
+        const int64_t bi = (w1 - 1) / p->n_seg, seg = (w1 - 1) % p->n_seg;
+        int64_t hi = seg * (int64_t)p->S - p->m / 2 + p->L;
+        if (hi > p->n_f) hi = p->n_f;
+        size_t upto = (size_t)bi * (size_t)p->n_f + (size_t)hi;
+        if (c == n_chunks - 1) upto = (size_t)p->n_batch * (size_t)p->n_f;
+        if (upto > copied) {
+            e = cudaMemcpyAsync((float2 *)p->d_host_spec + copied, (const float2 *)h_spectrum + copied, sizeof(float2) * (upto - copied),
+                                cudaMemcpyHostToDevice, p->copy_stream);
+            copied = upto;
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(p->copy_event[c], p->copy_stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, p->copy_event[c], 0);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        fdas_status s = enqueue(p, OUT_BLOCKMAX, p->d_host_spec, nullptr, nullptr, d_max, (int *)d_arg, cuda_stream, w0, w1);
+        if (s != FDAS_OK) return s;
+    }
+    p->last_launches = n_chunks;
     e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -602,6 +653,10 @@ fdas_status fdas_plan_destroy(fdas_plan *p)
     if (p->d_host_spec) cudaFree(p->d_host_spec);
     if (p->d_host_power) cudaFree(p->d_host_power);
     if (p->d_host_det) cudaFree(p->d_host_det);
+    if (p->copy_stream) {
+        for (int i = 0; i <= HOST_CHUNKS; ++i) if (p->copy_event[i]) cudaEventDestroy(p->copy_event[i]);
+        cudaStreamDestroy(p->copy_stream);
+    }
     (void)cudaGetLastError();
     free(p);
     return FDAS_OK;
