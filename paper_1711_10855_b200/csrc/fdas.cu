@@ -555,6 +555,15 @@ static cudaError_t stage_reserve(void **buf, size_t *have, size_t need)
     return e;
 }
 
+// the plan's copy stream and events of the *_host entry points, created on first use
+static cudaError_t ensure_copy_stream(fdas_plan *p)
+{
+    if (p->copy_stream) return cudaSuccess;
+    cudaError_t e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; e == cudaSuccess && i <= HOST_CHUNKS; ++i) e = cudaEventCreateWithFlags(&p->copy_event[i], cudaEventDisableTiming);
+    return e;
+}
+
 fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_power, void *cuda_stream)
 {
     if (!p || !h_spectrum || !h_power) return FDAS_ERR_INVALID_ARG;
@@ -568,9 +577,42 @@ fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_po
     cudaStream_t st = (cudaStream_t)cuda_stream;
     e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(p, e);
-    fdas_status s = fdas_convolve(p, p->d_host_spec, p->d_host_power, cuda_stream);
-    if (s != FDAS_OK) return s;
-    e = cudaMemcpyAsync(h_power, p->d_host_power, pb, cudaMemcpyDeviceToHost, st);
+    // The plane is 100 x the spectrum: its way back dominates.  The work items are launched in up to HOST_CHUNKS
+    // pieces of at least a wave each, and every piece's columns start their way back (2-D copies on the plan's copy
+    // stream) while the next piece is computed.
+    const int64_t n_work = p->n_seg * (int64_t)p->n_batch;
+    const int64_t waves = (n_work + p->grid_max[OUT_POWER] - 1) / p->grid_max[OUT_POWER];
+    const int n_chunks = (int)(waves > HOST_CHUNKS ? HOST_CHUNKS : waves);
+    if (n_chunks <= 1) {
+        fdas_status s = fdas_convolve(p, p->d_host_spec, p->d_host_power, cuda_stream);
+        if (s != FDAS_OK) return s;
+        e = cudaMemcpyAsync(h_power, p->d_host_power, pb, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        return FDAS_OK;
+    }
+    e = ensure_copy_stream(p);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    const size_t pitch = sizeof(float) * (size_t)p->n_f;
+    for (int c = 0; c < n_chunks; ++c) {
+        const int64_t w0 = n_work * c / n_chunks, w1 = n_work * (c + 1) / n_chunks;
+        fdas_status s = enqueue(p, OUT_POWER, p->d_host_spec, p->d_host_power, nullptr, nullptr, nullptr, cuda_stream, w0, w1);
+        if (s != FDAS_OK) return s;
+        e = cudaEventRecord(p->copy_event[c], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, p->copy_event[c], 0);
+        for (int64_t bi = w0 / p->n_seg; e == cudaSuccess && bi <= (w1 - 1) / p->n_seg; ++bi) { // batch items the piece touches
+            const int64_t sa = bi == w0 / p->n_seg ? w0 % p->n_seg : 0;
+            const int64_t sz = bi == (w1 - 1) / p->n_seg ? (w1 - 1) % p->n_seg + 1 : p->n_seg;
+            const int64_t c0 = sa * p->S, c1 = sz * p->S < p->n_f ? sz * p->S : p->n_f;
+            const size_t off = (size_t)bi * (size_t)p->n_z * (size_t)p->n_f + (size_t)c0;
+            e = cudaMemcpy2DAsync(h_power + off, pitch, p->d_host_power + off, pitch, sizeof(float) * (size_t)(c1 - c0), (size_t)p->n_z,
+                                  cudaMemcpyDeviceToHost, p->copy_stream);
+        }
+        if (e != cudaSuccess) return cuda_fail(p, e);
+    }
+    p->last_launches = n_chunks;
+    e = cudaEventRecord(p->copy_event[HOST_CHUNKS], p->copy_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, p->copy_event[HOST_CHUNKS], 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(p, e);
     return FDAS_OK;
@@ -608,11 +650,8 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, floa
         if (e != cudaSuccess) return cuda_fail(p, e);
         return FDAS_OK;
     }
-    if (!p->copy_stream) {
-        e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
-        for (int i = 0; e == cudaSuccess && i <= HOST_CHUNKS; ++i) e = cudaEventCreateWithFlags(&p->copy_event[i], cudaEventDisableTiming);
-        if (e != cudaSuccess) return cuda_fail(p, e);
-    }
+    e = ensure_copy_stream(p);
+    if (e != cudaSuccess) return cuda_fail(p, e);
     e = cudaEventRecord(p->copy_event[HOST_CHUNKS], st);                  // the copies start after the caller's earlier work
     if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, p->copy_event[HOST_CHUNKS], 0);
     if (e != cudaSuccess) return cuda_fail(p, e);
@@ -870,6 +909,6 @@ int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b)
 }
 
 // The kernel generation is what profiles/traffic.json is keyed by: bump it with every change to the hot kernel.
-const char *fdas_version(void) { return "libfdas sm_100a k7"; }
+const char *fdas_version(void) { return "libfdas sm_100a k8"; }
 
 } // extern "C"
