@@ -75,3 +75,28 @@ def test_no_cpu_fallback_without_a_gpu():
     with pytest.raises(B.FdasError) as e:
         B.Plan(1 << 12, 4, 2, 64, 512)
     assert e.value.status in (B.FDAS_ERR_CUDA, B.FDAS_ERR_ALLOC)
+
+
+def test_round2_entries_validate_before_touching_the_gpu():
+    """The entry points added in round 2: NULL handling and argument checks that need no device."""
+    L = B.lib()
+    assert L.fdas_convolve_complex(None, None, None, None) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_detect_blockmax(None, None, None, None, None) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_detect_blockmax_host(None, None, None, None, None) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_plan_set_symmetry(None, 1) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_plan_symmetry_active(None) == 0 and L.fdas_plan_grid(None) == 0
+    out = ctypes.c_void_p()
+    # stand-alone FFT: (n, elements per thread) combinations that do not exist
+    for n, e, status in [(1000, 0, B.FDAS_ERR_UNSUPPORTED), (256, 0, B.FDAS_ERR_UNSUPPORTED), (4096, 8, B.FDAS_ERR_UNSUPPORTED),
+                         (512, 16, B.FDAS_ERR_UNSUPPORTED), (1024, 4, B.FDAS_ERR_UNSUPPORTED)]:
+        assert L.fdas_fft_plan_create(ctypes.byref(out), n, e) == status and not out.value
+    assert L.fdas_fft_plan_create(None, 1024, 0) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_fft_exec(None, 1, 8, 16, 0, None) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_fft_plan_destroy(None) == B.FDAS_OK and L.fdas_fft_plan_grid(None) == 0
+    # spectrum step: sample counts that are not powers of two, or outside 2^19 .. 2^27
+    for n, status in [(0, B.FDAS_ERR_INVALID_ARG), (3 << 20, B.FDAS_ERR_INVALID_ARG), (1 << 18, B.FDAS_ERR_UNSUPPORTED),
+                      (1 << 28, B.FDAS_ERR_UNSUPPORTED)]:
+        assert L.fdas_spectrum_plan_create(ctypes.byref(out), n, 4096) == status and not out.value
+    assert L.fdas_spectrum_exec(None, None, None, None) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_spectrum_plan_destroy(None) == B.FDAS_OK and L.fdas_spectrum_plan_bins(None) == 0
+    assert L.fdas_debug_alu_peak(0, None, None) == B.FDAS_ERR_INVALID_ARG
