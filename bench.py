@@ -456,7 +456,8 @@ def run_fft(args):
            "variants": rows, "clocks": clocks, "gpu_launches": launches,
            "paper_context": "Table 1 (P:56-60): 1.80 ms on P100, 2.21 ms on TITAN X (Pascal) for 100 000 FFTs, N = 1024; other hardware, not a target",
            "roofline": {"bound": "hbm", "achieved": best["hbm_gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
-                        "frac": best["hbm_frac"], "traffic": None, "kernel": "fdas::fdas_fft_batch_kernel",
+                        "frac": best["hbm_frac"], "traffic": ncu_traffic(f"fft{n}e{best['elems_per_thread']}", binding.version())[0],
+                        "kernel": "fdas::fdas_fft_batch_kernel",
                         "bytes_per_launch": n_total * n * 16}}
     print(json.dumps(out))
     return 0
