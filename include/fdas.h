@@ -22,8 +22,9 @@
  * if none is usable.
  *
  * Conventions: "HOST" / "DEVICE" say where a pointer must live.  Complex data are interleaved
- * (re, im) float32 pairs.  No exception crosses this boundary; no global state; a plan may be used
- * from several host threads as long as calls on the same plan are not concurrent.
+ * (re, im) float32 pairs.  No exception crosses this boundary; no global state (one exception: the static device
+ * scratch of fdas_convolve_noalloc, described there); a plan may be used from several host threads as long as
+ * calls on the same plan are not concurrent.
  */
 #ifndef FDAS_H
 #define FDAS_H
@@ -42,7 +43,8 @@ typedef enum {
     FDAS_ERR_UNSUPPORTED = 2,  /* segment_len not in {512, 1024, 2048, 4096, 8192} */
     FDAS_ERR_ALLOC = 3,        /* host or device allocation failed */
     FDAS_ERR_NO_TEMPLATES = 4, /* fdas_convolve before fdas_set_templates */
-    FDAS_ERR_CUDA = 5          /* a CUDA runtime call failed; see fdas_plan_last_cuda_error */
+    FDAS_ERR_CUDA = 5,         /* a CUDA runtime call failed; see fdas_plan_last_cuda_error */
+    FDAS_ERR_TOO_LARGE = 6     /* fdas_convolve_noalloc: n_z * segment_len exceeds FDAS_NOALLOC_MAX_BANK */
 } fdas_status;
 
 /*
@@ -112,6 +114,63 @@ int fdas_plan_symmetry_active(const fdas_plan *plan);
  * Errors: INVALID_ARG (NULL / misaligned pointers), NO_TEMPLATES, CUDA (launch failure).
  */
 fdas_status fdas_convolve(fdas_plan *plan, const void *d_spectrum, float *d_power, void *cuda_stream);
+
+/*
+ * fdas_convolve for callers that must not allocate device memory: the whole of fdas_plan_create +
+ * fdas_set_templates + fdas_convolve in one call that never calls cudaMalloc, cudaFree or any routine that does.
+ *
+ * Who needs it.  Every other way into this library goes through a plan, and a plan is built from cudaMalloc calls
+ * (the transformed bank, the twiddle table, the work counters; fdas_set_templates adds a temporary).  Some hosts
+ * cannot afford that: a telescope back end that carved up the whole card when it started and keeps searching for
+ * days, where a cudaMalloc in the middle of the run stalls every stream of the device while the driver maps memory
+ * and can fail outright because nothing is left; a process in which a framework's pool allocator already holds
+ * the free memory, so the driver has none to give although the pool has plenty; code that is handed its buffers
+ * and is forbidden by its own rules to take more (fixed memory budgets, certification, a callback that runs while
+ * other work is in flight).  Such a caller passes its inputs and its output as usual, and the memory the kernels
+ * need besides them comes out of the library image instead.
+ *
+ * Where the scratch lives.  libfdas.so carries one file-scope __device__ array of FDAS_NOALLOC_SCRATCH_BYTES
+ * (8 MiB + 64 KiB + 256 B).  The CUDA runtime gives every GPU that loads the library its own copy when the
+ * library's device code is loaded there and keeps it until the process exits, whether this entry point is ever
+ * called or not.  It holds, in this order, the two work counters of the persistent kernel, the twiddle table
+ * w_L^j (eq.(3); 8192 entries at most) and the transformed template bank (n_z * L complex64).  The bank is
+ * what sets THE LIMIT: n_z * segment_len <= FDAS_NOALLOC_MAX_BANK = 2^20 elements, enough for every
+ * BASELINE.json configuration (config 3: 201 * 4096 = 823 296).  A larger request is refused with
+ * FDAS_ERR_TOO_LARGE before anything is launched; use a plan for those.
+ *
+ * What a call does, all on cuda_stream and in this order: (1) one small kernel writes the twiddle table for this
+ * segment_len and sets the work counters to zero; (2) the template kernel of fdas_set_templates conjugates, pads,
+ * scales and transforms the taps into the scratch bank; (3) the hot kernel of fdas_convolve runs exactly as it does
+ * for a plan.  Nothing is kept between calls on purpose: the array still holds whatever the previous call left
+ * (another bank, the table of another segment length, counters of a launch that was aborted), so every call
+ * rewrites all of what it reads and clears the counters itself.  The price is the template transform on every
+ * call, n_z of the (1 + n_z) * n_seg transforms -- 0.1 % on config 3.
+ *
+ *   n_f, z_max, z_step, template_width, segment_len   as fdas_plan_create (same checks, same errors)
+ *   n_batch       >= 1, as fdas_plan_set_batch
+ *   d_templates   DEVICE, float32 [n_z][m][2] as in fdas_set_templates but already on the GPU, 8-byte aligned,
+ *                 read only (the caller owns it; a host pointer here faults inside the kernel)
+ *   d_spectrum, d_power, cuda_stream   as fdas_convolve
+ * Asynchronous.  The result equals fdas_convolve's to rounding (the twiddle table is evaluated on the GPU here and
+ * on the host there; the two could differ in the last bit of an entry -- on the shapes of
+ * tests/test_zz_no_alloc.py they do not, and the planes agree bit for bit).
+ *
+ * All calls on one GPU share the one array.  Two calls whose GPU work overlaps -- different streams, or different
+ * host threads -- overwrite each other's bank and counters and both results are garbage without any error being
+ * reported: put them on one stream or order them with events.  Calls on different GPUs are independent.
+ *
+ * First call on each GPU: besides the above it looks up the device address of the array (cudaGetSymbolAddress,
+ * with that GPU current) and raises the kernels' shared-memory limits (cudaFuncSetAttribute).  These are host-side
+ * set-up calls, not stream work.  Make this first call before you begin any stream capture on that GPU.
+ * Thread safe with respect to that set-up; at most 64 GPUs per process (more: FDAS_ERR_UNSUPPORTED).
+ * Errors: INVALID_ARG, UNSUPPORTED, TOO_LARGE as described (all three are decided before the first CUDA call);
+ * CUDA if the set-up or a launch fails (the runtime's error state has been cleared by then; there is no plan to
+ * ask for the code).
+ */
+#define FDAS_NOALLOC_MAX_BANK (1 << 20)                                   /* complex64 elements: n_z * segment_len */
+#define FDAS_NOALLOC_SCRATCH_BYTES (256 + 8 * 8192 + 8 * FDAS_NOALLOC_MAX_BANK)
+fdas_status fdas_convolve_noalloc(int64_t n_f, int n_batch, int z_max, int z_step, int template_width, int segment_len,
+                                  const float *d_templates, const void *d_spectrum, float *d_power, void *cuda_stream);
 
 /*
  * Convenience for callers whose data live in HOST memory (bench.py's "e2e" leg): copies

@@ -13,6 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libfdas.so")
 
 FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_UNSUPPORTED, FDAS_ERR_ALLOC, FDAS_ERR_NO_TEMPLATES, FDAS_ERR_CUDA = range(6)
+FDAS_ERR_TOO_LARGE = 6
+NOALLOC_MAX_BANK = 1 << 20  # FDAS_NOALLOC_MAX_BANK: n_z * segment_len that fdas_convolve_noalloc accepts
 
 # every symbol include/fdas.h declares: name -> (restype, argtypes)
 _vp, _i64, _int = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
@@ -23,6 +25,7 @@ SYMBOLS = {
     "fdas_plan_set_symmetry": (_int, [_vp, _int]),
     "fdas_plan_symmetry_active": (_int, [_vp]),
     "fdas_convolve": (_int, [_vp, _vp, _vp, _vp]),
+    "fdas_convolve_noalloc": (_int, [_i64, _int, _int, _int, _int, _int, _vp, _vp, _vp, _vp]),
     "fdas_convolve_host": (_int, [_vp, _vp, _vp, _vp]),
     "fdas_convolve_complex": (_int, [_vp, _vp, _vp, _vp]),
     "fdas_detect_blockmax": (_int, [_vp, _vp, _vp, _vp, _vp]),
@@ -244,6 +247,19 @@ class SpectrumPlan:
             self.destroy()
         except Exception:
             pass
+
+
+def convolve_noalloc(n_f, n_batch, z_max, z_step, template_width, segment_len, d_templates, d_spectrum, d_power, stream=None):
+    """fdas_convolve_noalloc: plan-less fdas_convolve that allocates nothing (scratch inside libfdas.so).
+
+    For hosts that cannot call cudaMalloc while they run (all device memory handed out at start-up, or owned by a
+    framework's pool).  d_templates: DEVICE complex64 [n_z][m]; the other buffers as Plan.convolve.  Raises
+    FdasError(FDAS_ERR_TOO_LARGE) when n_z * segment_len > NOALLOC_MAX_BANK.  Calls on one GPU share one scratch
+    array: keep them on one stream.  Make the first call on a GPU outside any stream capture.
+    """
+    _check(lib().fdas_convolve_noalloc(int(n_f), int(n_batch), int(z_max), int(z_step), int(template_width), int(segment_len),
+                                       _ptr(d_templates), _ptr(d_spectrum), _ptr(d_power), _stream(stream)),
+           "fdas_convolve_noalloc")
 
 
 def debug_fft(segment_len, n_seg, d_in, d_out, inverse=False):

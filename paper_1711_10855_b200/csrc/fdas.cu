@@ -16,6 +16,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "../../include/fdas.h"
 #include "fft_device.cuh"
 #include "convolve.cuh"
@@ -848,6 +850,7 @@ const char *fdas_status_string(fdas_status s)
     case FDAS_ERR_ALLOC: return "FDAS_ERR_ALLOC";
     case FDAS_ERR_NO_TEMPLATES: return "FDAS_ERR_NO_TEMPLATES";
     case FDAS_ERR_CUDA: return "FDAS_ERR_CUDA";
+    case FDAS_ERR_TOO_LARGE: return "FDAS_ERR_TOO_LARGE";
     }
     return "FDAS_ERR_UNKNOWN";
 }
@@ -907,6 +910,158 @@ int64_t fdas_debug_layout(int segment_len, int what, int t, int a, int b)
     FDAS_DISPATCH_L(segment_len, r = layout_query<LL>(what, t, a, b));
     return r;
 }
+
+} // extern "C"
+
+// -------------------------------------------------------------------------------------------
+// fdas_convolve_noalloc: the plan-less entry point for callers that may not allocate device memory
+// (include/fdas.h says who they are).  Everything a plan would have cudaMalloc'ed -- work counters, twiddle
+// table, transformed bank -- sits in ONE array that is part of the library image, so the CUDA runtime
+// places a copy on every GPU that loads libfdas.so and no call here ever asks the driver for memory.
+//
+// The name `noalloc_scratch` means two different things.  Inside device code it is the array.  Inside host
+// code it is only a handle the runtime knows the array by: handing `noalloc_scratch` itself to a kernel
+// passes a HOST address (a fault on the GPU, or on machines where the GPU can read host memory a quiet
+// scribble over host data).  Host code therefore asks the runtime for the device address, once per GPU
+// and with that GPU current (noalloc_device below), and gives the kernels that.
+// -------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char noalloc_scratch[FDAS_NOALLOC_SCRATCH_BYTES];
+
+namespace fdas {
+// Part (1) of a call: w_L^j = exp(-i 2 pi j / L) for this L (evaluated in double, rounded once, like the host
+// table of a plan) and the two work counters back to zero -- whatever the previous call, or a launch
+// that never finished, left in them.
+__global__ void __launch_bounds__(256) fdas_noalloc_init_kernel(float2 *__restrict__ tw, int L, unsigned int *__restrict__ work)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < L) {
+        double s, c;
+        sincospi(-2.0 * (double)j / (double)L, &s, &c);
+        tw[j] = make_float2((float)c, (float)s);
+    }
+    if (j == 0) { work[0] = 0u; work[1] = 0u; }
+}
+} // namespace fdas
+
+namespace {
+
+constexpr size_t NOALLOC_WORK_OFF = 0, NOALLOC_TW_OFF = 256, NOALLOC_BANK_OFF = 256 + 8 * 8192;
+static_assert(NOALLOC_BANK_OFF + 8 * (size_t)FDAS_NOALLOC_MAX_BANK == FDAS_NOALLOC_SCRATCH_BYTES, "scratch layout");
+constexpr int NOALLOC_MAX_DEVICES = 64;
+
+struct NoallocDevice {
+    bool ready;
+    unsigned char *base; // DEVICE address of noalloc_scratch on this GPU
+    int grid_max[5];     // persistent grid of the power kernel for L = 512 << i
+};
+NoallocDevice noalloc_dev[NOALLOC_MAX_DEVICES];
+std::mutex noalloc_mutex;
+
+int noalloc_L_index(int L) { return L == 512 ? 0 : L == 1024 ? 1 : L == 2048 ? 2 : L == 4096 ? 3 : 4; }
+
+template <int L> cudaError_t noalloc_prepare(int dev, int *grid_max)
+{
+    cudaError_t e = prepare_convolve<L, OUT_POWER>(dev, grid_max);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(fdas_template_fft_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<L>());
+    return e;
+}
+
+// part (2) of a call: fdas_set_templates' kernel, but on the caller's stream and writing the scratch bank
+template <int L> cudaError_t noalloc_bank(const float2 *d_h, int m, int n_z, const float2 *tw, float4 *bank, cudaStream_t st)
+{
+    fdas_template_fft_kernel<L><<<(unsigned)n_z, Cfg<L>::NT, smem_bytes<L>(), st>>>(d_h, m, tw, bank);
+    return cudaGetLastError();
+}
+
+// First call on a GPU (that GPU is current): device address of the array, opt-in shared-memory sizes of the two
+// kernels for every segment length, grid sizes.  Host-side calls only; nothing is allocated, nothing enqueued.
+cudaError_t noalloc_device(int dev, const NoallocDevice **out)
+{
+    std::lock_guard<std::mutex> lock(noalloc_mutex);
+    NoallocDevice &d = noalloc_dev[dev];
+    if (!d.ready) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, noalloc_scratch);
+        if (e == cudaSuccess && (ptr == nullptr || ((uintptr_t)ptr & 255u))) e = cudaErrorInvalidSymbol;
+        if (e != cudaSuccess) return e;
+        int L = 512;
+        for (int i = 0; i < 5 && e == cudaSuccess; ++i, L *= 2) { FDAS_DISPATCH_L(L, (e = noalloc_prepare<LL>(dev, &d.grid_max[i]))); }
+        if (e != cudaSuccess) return e;
+        d.base = (unsigned char *)ptr;
+        d.ready = true;
+    }
+    *out = &d;
+    return cudaSuccess;
+}
+
+} // namespace
+
+extern "C" fdas_status fdas_convolve_noalloc(int64_t n_f, int n_batch, int z_max, int z_step, int template_width, int segment_len,
+                                             const float *d_templates, const void *d_spectrum, float *d_power, void *cuda_stream)
+{
+    // the argument rules of fdas_plan_create / fdas_plan_set_batch / fdas_convolve
+    if (n_f < 1 || n_batch < 1 || z_max < 0 || z_step < 1 || (z_max % z_step) != 0) return FDAS_ERR_INVALID_ARG;
+    if (template_width < 2 || (template_width & 1)) return FDAS_ERR_INVALID_ARG;
+    if (segment_len < 2 || (segment_len & (segment_len - 1))) return FDAS_ERR_INVALID_ARG;
+    if (!supported_L(segment_len)) return FDAS_ERR_UNSUPPORTED;
+    if (template_width > segment_len / 2) return FDAS_ERR_INVALID_ARG;
+    if (!d_templates || !d_spectrum || !d_power) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_templates & 7u) || ((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_power & 3u)) return FDAS_ERR_INVALID_ARG;
+    const int L = segment_len, m = template_width;
+    const int64_t n_z = 2 * (int64_t)(z_max / z_step) + 1;
+    // the one limit of this entry point: the transformed bank has to fit its part of the static array
+    if (n_z * (int64_t)L > (int64_t)FDAS_NOALLOC_MAX_BANK) return FDAS_ERR_TOO_LARGE;
+
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return FDAS_ERR_UNSUPPORTED;
+    const NoallocDevice *d = nullptr;
+    e = noalloc_device(dev, &d);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+
+    unsigned int *work = (unsigned int *)(d->base + NOALLOC_WORK_OFF);
+    float2 *tw = (float2 *)(d->base + NOALLOC_TW_OFF);
+    float4 *bank = (float4 *)(d->base + NOALLOC_BANK_OFF);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    // (1) twiddle table of this L, counters to zero
+    fdas_noalloc_init_kernel<<<(L + 255) / 256, 256, 0, st>>>(tw, L, work);
+    e = cudaGetLastError();
+    // (2) the bank: conj, pad, 1/L, forward transform, register order (fdas_set_templates' kernel, on the caller's stream)
+    if (e == cudaSuccess) {
+        e = cudaErrorInvalidValue;
+        FDAS_DISPATCH_L(L, (e = noalloc_bank<LL>((const float2 *)d_templates, m, (int)n_z, tw, bank, st)));
+    }
+    // (3) the hot kernel, as fdas_convolve launches it
+    if (e == cudaSuccess) {
+        ConvParams cp;
+        cp.spectrum = (const float2 *)d_spectrum;
+        cp.power = d_power;
+        cp.amp = nullptr;
+        cp.bmax = nullptr;
+        cp.barg = nullptr;
+        cp.gperm = bank;
+        cp.tw = tw;
+        cp.work = work;
+        cp.n_f = n_f;
+        cp.S = L - m;
+        cp.n_seg = (n_f + cp.S - 1) / cp.S;
+        cp.n_work = cp.n_seg * (int64_t)n_batch;
+        cp.w_begin = 0;
+        cp.n_z = (int)n_z;
+        cp.m = m;
+        cp.bulk_ok = ((uintptr_t)d_spectrum & 15u) == 0;
+        const int gmax = d->grid_max[noalloc_L_index(L)];
+        e = cudaErrorInvalidValue;
+        FDAS_DISPATCH_L(L, (e = launch_convolve<LL, OUT_POWER>(cp, gmax, st)));
+    }
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    return FDAS_OK;
+}
+
+extern "C" {
 
 // The kernel generation is what profiles/traffic.json is keyed by: bump it with every change to the hot kernel.
 const char *fdas_version(void) { return "libfdas sm_100a k8"; }
