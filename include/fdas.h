@@ -24,7 +24,8 @@
  * Conventions: "HOST" / "DEVICE" say where a pointer must live.  Complex data are interleaved
  * (re, im) float32 pairs.  No exception crosses this boundary; no global state (one exception: the static device
  * scratch of fdas_convolve_noalloc, described there); a plan may be used from several host threads as long as
- * calls on the same plan are not concurrent.
+ * calls on the same plan are not concurrent (the asynchronous launches fdas_convolve, fdas_convolve_complex and
+ * fdas_detect_blockmax are the exception: see fdas_convolve).
  */
 #ifndef FDAS_H
 #define FDAS_H
@@ -108,8 +109,10 @@ int fdas_plan_symmetry_active(const fdas_plan *plan);
  * Asynchronous: only launches; never synchronises, allocates or copies.  The buffers must stay
  * valid until the stream has run the work.  Output is bitwise reproducible (the kernel hands out
  * segments through an atomic counter, but which CTA computes a segment does not change its result).
- * The plan may be used from several streams at once; at most 1024 launches of one plan may be
- * in flight (enqueued and not finished) at any time: they take the plan's work counters round robin.
+ * The plan may be used from several streams at once, also from several host threads (one stream each; the
+ * counter hand-out is atomic); at most 1024 launches of one plan may be in flight (enqueued and not finished)
+ * at any time: they take the plan's work counters round robin.  fdas_plan_last_launch_count then reports on
+ * whichever call wrote last.
  * Must be called with the plan's device current (the one current at fdas_plan_create).
  * Errors: INVALID_ARG (NULL / misaligned pointers), NO_TEMPLATES, CUDA (launch failure).
  */
@@ -175,7 +178,8 @@ fdas_status fdas_convolve_noalloc(int64_t n_f, int n_batch, int z_max, int z_ste
 /*
  * Convenience for callers whose data live in HOST memory (bench.py's "e2e" leg): copies
  * h_spectrum to a plan-owned device buffer, runs fdas_convolve, copies the power plane back to
- * h_power, and synchronises the stream.  Buffers are allocated on first use and kept by the plan:
+ * h_power, and synchronises the stream.  On an error return, too, nothing is left in flight that touches
+ * h_spectrum or h_power (the call waits for what it had enqueued): the caller may free them at once.  Buffers are allocated on first use and kept by the plan:
  * two *_host calls on one plan must not overlap (not from two host threads, not on two streams).
  *   h_spectrum    HOST (pinned memory gives asynchronous copies), complex64 [n_batch][n_f]
  *   h_power       HOST, float32 [n_batch][n_z][n_f]
@@ -223,7 +227,10 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *plan, const void *h_spectrum, f
 typedef struct fdas_fft_plan fdas_fft_plan;
 fdas_status fdas_fft_plan_create(fdas_fft_plan **out, int n, int elems_per_thread);
 fdas_status fdas_fft_exec(fdas_fft_plan *plan, int64_t n_fft, const void *d_in, void *d_out, int inverse, void *cuda_stream);
-/* The repetition scheme of P:46: n_launches identical launches of n_fft transforms each, enqueued back to back. */
+/* The repetition scheme of P:46: n_launches launches of n_fft transforms each, enqueued back to back.  Launch i
+ * transforms sequences [i*n_fft, (i+1)*n_fft), so d_in and d_out are DEVICE complex64 [n_launches * n_fft][n] and the
+ * 1000 x 100 protocol reads and writes 100 000 distinct sequences (from and to HBM), the same data as one launch of
+ * 100 000. */
 fdas_status fdas_fft_exec_many(fdas_fft_plan *plan, int n_launches, int64_t n_fft, const void *d_in, void *d_out,
                                int inverse, void *cuda_stream);
 fdas_status fdas_fft_plan_destroy(fdas_fft_plan *plan);

@@ -29,7 +29,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", LIB + ".tmp"] + sources()
+    # FDAS_BUILD_EXPERIMENTS=1 compiles the experiment knobs in (FDAS_EXP_GRID, FDAS_EXP_NOBULK: grid sweeps and the
+    # guarded-load path for profiles/); the shipped library has none and never reads the environment
+    extra = ["-DFDAS_EXPERIMENTS"] if os.environ.get("FDAS_BUILD_EXPERIMENTS") else []
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", LIB + ".tmp"] + sources()
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB

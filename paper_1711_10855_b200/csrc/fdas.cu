@@ -135,6 +135,9 @@ struct fdas_plan {
     bool sym_detected;        // the current bank satisfies h_{-z} = conj(h_{+z}) bit for bit
     unsigned int *d_work;     // [WORK_SLOTS][2] work counters of the persistent kernel, zero between launches
     unsigned int work_seq;    // launches so far: selects the counter pair
+#ifdef FDAS_EXPERIMENTS
+    bool exp_nobulk;          // FDAS_EXP_NOBULK was set when the plan was created
+#endif
     // buffers of fdas_convolve_host
     void *d_host_spec;
     float *d_host_power;
@@ -232,8 +235,15 @@ template <int L, int OUT, bool SYM = false> cudaError_t prepare_convolve(int dev
     if (per_sm > 512 / TmemCfg<Cfg<L>>::NCOLS) per_sm = 512 / TmemCfg<Cfg<L>>::NCOLS;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *grid_max = per_sm * n_sm;
-    // experiment knob (profiles/r2_c3_k6.md, r2_all_configs.md: grid-size sweeps); not part of the interface
-    if (const char *g = getenv("FDAS_EXP_GRID")) *grid_max = atoi(g);
+#ifdef FDAS_EXPERIMENTS
+    // experiment knob (profiles/r2_c3_k6.md, r2_all_configs.md: grid-size sweeps); compiled out of the shipped library
+    // (build.py never defines FDAS_EXPERIMENTS).  Read once per plan, at creation; values outside 1 .. resident CTAs
+    // are ignored: 0 would launch an empty grid, more CTAs than fit would break the persistent kernel's one-wave rule.
+    if (const char *g = getenv("FDAS_EXP_GRID")) {
+        const long v = strtol(g, nullptr, 10);
+        if (v >= 1 && v <= (long)*grid_max) *grid_max = (int)v;
+    }
+#endif
     return cudaSuccess;
 }
 
@@ -401,6 +411,9 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t n_f, int z_max, int z_step
     p->S = segment_len - template_width;
     p->n_seg = (n_f + p->S - 1) / p->S;
     p->n_batch = 1;
+#ifdef FDAS_EXPERIMENTS
+    p->exp_nobulk = getenv("FDAS_EXP_NOBULK") != nullptr;
+#endif
     cudaError_t e = cudaGetDevice(&p->device);
     if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_gperm, sizeof(float2) * (size_t)p->n_z * (size_t)p->L);
     if (e == cudaSuccess) e = upload_twiddles(p->L, &p->d_tw);
@@ -493,7 +506,9 @@ static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, f
     cp.barg = d_arg;
     cp.gperm = p->d_gperm;
     cp.tw = p->d_tw;
-    cp.work = p->d_work + 2 * (p->work_seq++ % WORK_SLOTS);
+    // fetch-and-add: launches on one plan may come from several host threads (one stream each), and two of them must
+    // never be handed the same counter pair
+    cp.work = p->d_work + 2 * (__atomic_fetch_add(&p->work_seq, 1u, __ATOMIC_RELAXED) % WORK_SLOTS);
     cp.n_f = p->n_f;
     cp.n_seg = p->n_seg;
     cp.n_work = w_end >= 0 ? w_end : p->n_seg * (int64_t)p->n_batch;
@@ -502,7 +517,9 @@ static fdas_status enqueue(fdas_plan *p, int out_mode, const void *d_spectrum, f
     cp.m = p->m;
     cp.S = p->S;
     cp.bulk_ok = ((uintptr_t)d_spectrum & 15u) == 0;
-    if (getenv("FDAS_EXP_NOBULK")) cp.bulk_ok = 0; // experiment knob: guarded loads for every segment
+#ifdef FDAS_EXPERIMENTS
+    if (p->exp_nobulk) cp.bulk_ok = 0; // experiment knob (read at plan creation): guarded loads for every segment
+#endif
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaErrorInvalidValue;
     const int L = p->L;
@@ -557,6 +574,16 @@ static cudaError_t stage_reserve(void **buf, size_t *have, size_t need)
     return e;
 }
 
+// A *_host call that fails after it has enqueued something: kernels may still be queued on the caller's stream and
+// copies from / into the caller's HOST buffers on the plan's copy stream.  The caller is entitled to free those buffers
+// as soon as the error comes back, so wait for both streams first (their own status no longer matters).
+static void host_drain(fdas_plan *p, cudaStream_t st)
+{
+    if (p->copy_stream) (void)cudaStreamSynchronize(p->copy_stream);
+    (void)cudaStreamSynchronize(st);
+    (void)cudaGetLastError();
+}
+
 // the plan's copy stream and events of the *_host entry points, created on first use
 static cudaError_t ensure_copy_stream(fdas_plan *p)
 {
@@ -579,6 +606,7 @@ fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_po
     cudaStream_t st = (cudaStream_t)cuda_stream;
     e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(p, e);
+    // From here on work is in flight: every error return drains it first (host_drain).
     // The plane is 100 x the spectrum: its way back dominates.  The work items are launched in up to HOST_CHUNKS
     // pieces of at least a wave each, and every piece's columns start their way back (2-D copies on the plan's copy
     // stream) while the next piece is computed.
@@ -587,19 +615,19 @@ fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_po
     const int n_chunks = (int)(waves > HOST_CHUNKS ? HOST_CHUNKS : waves);
     if (n_chunks <= 1) {
         fdas_status s = fdas_convolve(p, p->d_host_spec, p->d_host_power, cuda_stream);
-        if (s != FDAS_OK) return s;
+        if (s != FDAS_OK) { host_drain(p, st); return s; }
         e = cudaMemcpyAsync(h_power, p->d_host_power, pb, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) return cuda_fail(p, e);
+        if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
         return FDAS_OK;
     }
     e = ensure_copy_stream(p);
-    if (e != cudaSuccess) return cuda_fail(p, e);
+    if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
     const size_t pitch = sizeof(float) * (size_t)p->n_f;
     for (int c = 0; c < n_chunks; ++c) {
         const int64_t w0 = n_work * c / n_chunks, w1 = n_work * (c + 1) / n_chunks;
         fdas_status s = enqueue(p, OUT_POWER, p->d_host_spec, p->d_host_power, nullptr, nullptr, nullptr, cuda_stream, w0, w1);
-        if (s != FDAS_OK) return s;
+        if (s != FDAS_OK) { host_drain(p, st); return s; }
         e = cudaEventRecord(p->copy_event[c], st);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, p->copy_event[c], 0);
         for (int64_t bi = w0 / p->n_seg; e == cudaSuccess && bi <= (w1 - 1) / p->n_seg; ++bi) { // batch items the piece touches
@@ -610,13 +638,13 @@ fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_po
             e = cudaMemcpy2DAsync(h_power + off, pitch, p->d_host_power + off, pitch, sizeof(float) * (size_t)(c1 - c0), (size_t)p->n_z,
                                   cudaMemcpyDeviceToHost, p->copy_stream);
         }
-        if (e != cudaSuccess) return cuda_fail(p, e);
+        if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
     }
     p->last_launches = n_chunks;
     e = cudaEventRecord(p->copy_event[HOST_CHUNKS], p->copy_stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, p->copy_event[HOST_CHUNKS], 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return cuda_fail(p, e);
+    if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
     return FDAS_OK;
 }
 
@@ -645,18 +673,18 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, floa
         e = cudaMemcpyAsync(p->d_host_spec, h_spectrum, sb, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return cuda_fail(p, e);
         fdas_status s1 = fdas_detect_blockmax(p, p->d_host_spec, d_max, d_arg, cuda_stream);
-        if (s1 != FDAS_OK) return s1;
+        if (s1 != FDAS_OK) { host_drain(p, st); return s1; }
         e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) return cuda_fail(p, e);
+        if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
         return FDAS_OK;
     }
     e = ensure_copy_stream(p);
     if (e != cudaSuccess) return cuda_fail(p, e);
     e = cudaEventRecord(p->copy_event[HOST_CHUNKS], st);                  // the copies start after the caller's earlier work
     if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, p->copy_event[HOST_CHUNKS], 0);
-    if (e != cudaSuccess) return cuda_fail(p, e);
+    if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
     size_t copied = 0; // complex elements of the flattened [n_batch][n_f] spectrum on the device so far
     for (int c = 0; c < n_chunks; ++c) {
         const int64_t w0 = n_work * c / n_chunks, w1 = n_work * (c + 1) / n_chunks;
@@ -673,15 +701,15 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, floa
         }
         if (e == cudaSuccess) e = cudaEventRecord(p->copy_event[c], p->copy_stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(st, p->copy_event[c], 0);
-        if (e != cudaSuccess) return cuda_fail(p, e);
+        if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
         fdas_status s = enqueue(p, OUT_BLOCKMAX, p->d_host_spec, nullptr, nullptr, d_max, (int *)d_arg, cuda_stream, w0, w1);
-        if (s != FDAS_OK) return s;
+        if (s != FDAS_OK) { host_drain(p, st); return s; }
     }
     p->last_launches = n_chunks;
     e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return cuda_fail(p, e);
+    if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
     return FDAS_OK;
 }
 
@@ -751,9 +779,11 @@ fdas_status fdas_fft_exec(fdas_fft_plan *p, int64_t n_fft, const void *d_in, voi
 fdas_status fdas_fft_exec_many(fdas_fft_plan *p, int n_launches, int64_t n_fft, const void *d_in, void *d_out, int inverse,
                                void *cuda_stream)
 {
-    if (n_launches < 0) return FDAS_ERR_INVALID_ARG;
+    if (!p || n_launches < 0 || n_fft < 0) return FDAS_ERR_INVALID_ARG;
+    // launch i transforms sequences [i * n_fft, (i+1) * n_fft): 1000 x 100 walks 100 000 distinct sequences through HBM
+    const size_t stride = (size_t)n_fft * (size_t)p->n;   // complex64 elements per launch
     for (int i = 0; i < n_launches; ++i) {
-        fdas_status s = fdas_fft_exec(p, n_fft, d_in, d_out, inverse, cuda_stream);
+        fdas_status s = fdas_fft_exec(p, n_fft, (const float2 *)d_in + i * stride, (float2 *)d_out + i * stride, inverse, cuda_stream);
         if (s != FDAS_OK) return s;
     }
     return FDAS_OK;

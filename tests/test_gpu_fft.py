@@ -82,3 +82,22 @@ def test_batched_fft_arguments():
         plan.exec(4, buf, buf)              # in place is not supported
     plan.exec(0, buf, torch.empty_like(buf))  # empty batch: nothing to do
     plan.destroy()
+
+
+def test_exec_many_walks_the_buffers():
+    """fdas_fft_exec_many ("100 FFTs per kernel launch, while launching 1000 of these kernels"): launch i
+    transforms sequences [i*n_fft, (i+1)*n_fft), so the protocol equals one launch over all of them, bit for bit."""
+    import torch
+    from paper_1711_10855_b200 import binding
+    n, n_launches, per = 1024, 7, 13
+    g = torch.Generator(device="cuda").manual_seed(46)
+    x = torch.randn((n_launches * per, n, 2), device="cuda", generator=g)
+    plan = binding.FftPlan(n)
+    y_one = torch.full_like(x, float("nan"))
+    y_many = torch.full_like(x, float("nan"))
+    plan.exec(n_launches * per, x, y_one)
+    plan.exec_many(n_launches, per, x, y_many)
+    torch.cuda.synchronize()
+    assert torch.isfinite(y_many).all()
+    assert torch.equal(y_one, y_many)
+    plan.destroy()
