@@ -91,20 +91,28 @@ def test_c3_block_maxima_every_row(torch, binding, oracle):
     wl = workload.make_config(3)
     gmax, garg, blk = _gpu_blockmax(wl, torch, binding)
     H = wl.templates.astype(np.complex128)
-    pmax = float(gmax.max())
-    tol = ABS_TOL * pmax
+    # The tolerance scales with the ORACLE's plane maximum, which is only known once all rows have been streamed:
+    # first pass keeps, per row chunk, the largest maximum error and the near-tie margins; they are judged at the end.
+    pmax_ref = 0.0
+    worst_err = 0.0
+    margins = []   # rmax - ref at the GPU's argmax, for every entry whose argmax differs from the oracle's
     n_same = n_all = 0
     for r0 in range(0, wl.n_z, 12):
         r1 = min(wl.n_z, r0 + 12)
         ref = oracle.ols(wl.spectrum[0], H, wl.seg_len, rows=(r0, r1))
+        pmax_ref = max(pmax_ref, float(ref.max()))
         rmax, rarg = oracle.blockmax(ref, blk)
         g, a = gmax[0][r0:r1], garg[0][r0:r1]
-        assert np.abs(g.astype(np.float64) - rmax).max() <= tol
+        worst_err = max(worst_err, float(np.abs(g.astype(np.float64) - rmax).max()))
         same = a == rarg
         n_same += int(same.sum()); n_all += same.size
         rr, bb = np.nonzero(~same)
         for r, b in zip(rr, bb):
-            assert ref[r, b * blk + a[r, b]] >= rmax[r, b] - 2 * tol, (r0 + r, b)
-    assert float(pmax) >= 0.99 * float(gmax.max())
+            margins.append(float(rmax[r, b] - ref[r, b * blk + a[r, b]]))
+    tol = ABS_TOL * pmax_ref
+    assert worst_err <= tol, (worst_err, tol)
+    assert all(mg <= 2 * tol for mg in margins), (max(margins), tol)
+    # the largest block maximum is the plane's maximum: the GPU's agrees with the oracle's
+    assert abs(float(gmax.max()) - pmax_ref) <= tol
     assert n_same / n_all > 0.999
     print(f"C3 block maxima: {n_same} of {n_all} argmax entries identical, the others near-ties")
