@@ -37,8 +37,8 @@ TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
 
 def ncu_traffic(workload_name, kernel_version):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the hot kernel from the committed
-    `ncu --set full` capture of THIS kernel version (profiles/traffic.json, written by hand from the
-    capture named there).  None when the library's kernel version has no capture: a stale figure is
+    `ncu --set full` capture of THIS kernel version (profiles/traffic.json: either a pointer to the tracked
+    raw export of the capture, read here, or for older generations numbers transcribed from it).  None when the library's kernel version has no capture: a stale figure is
     worse than none."""
     try:
         with open(TRAFFIC_JSON) as f:
@@ -48,6 +48,19 @@ def ncu_traffic(workload_name, kernel_version):
     e = table.get(kernel_version, {}).get(workload_name)
     if not e:
         return None, None
+    if "raw_csv" in e:  # the tracked raw export of the capture: header row, unit row, one row per profiled launch
+        try:
+            import csv
+            with open(os.path.join(os.path.dirname(TRAFFIC_JSON), os.path.basename(e["raw_csv"]))) as f:
+                rows = list(csv.reader(f))
+            col = {name: i for i, name in enumerate(rows[0])}
+            unit = rows[1]
+            rd, wr = col["dram__bytes_read.sum"], col["dram__bytes_write.sum"]
+            if unit[rd] != "byte" or unit[wr] != "byte":
+                return None, None
+            return int(float(rows[2][rd])) + int(float(rows[2][wr])), e["raw_csv"]
+        except (OSError, KeyError, IndexError, ValueError):
+            return None, None
     return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"]), e.get("source")
 
 
