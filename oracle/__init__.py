@@ -166,6 +166,25 @@ def blockmax(power, blk, float32_decision=True):
     return mx, ar
 
 
+def candidates(power, blk, threshold, capacity):
+    """Thresholded candidate list over a power plane [rows][cols] (reading 20; "detect"):
+    every block maximum of reading 17 whose float32 power is >= float32(threshold) is a candidate
+    (row, column = block * blk + offset, power as the float32 value the plane holds).  The list is ordered by (row, column); the first `capacity`
+    entries are kept.  Returns (n_found, rows int64 [n_kept], cols int64 [n_kept], powers float64 [n_kept]);
+    n_found counts every candidate, kept or not (n_found - n_kept is the overflow).
+    Written out step by step on top of blockmax: threshold, order, truncate."""
+    mx, ar = blockmax(power, blk, float32_decision=True)
+    thr = np.float32(threshold)
+    found = []
+    for r in range(mx.shape[0]):            # rows in order, blocks in order: (row, column) ascending
+        for b in range(mx.shape[1]):
+            if np.float32(mx[r, b]) >= thr:
+                found.append((r, b * int(blk) + int(ar[r, b]), float(mx[r, b])))
+    kept = found[:max(0, int(capacity))]
+    return (len(found), np.array([k[0] for k in kept], dtype=np.int64), np.array([k[1] for k in kept], dtype=np.int64),
+            np.array([k[2] for k in kept], dtype=np.float64))
+
+
 def spectrum(series, whiten_block=0):
     """P:21 "the FFT output of the observation" (reading 18): eq.(3) of the real series, bins
     0 .. n_t/2 - 1, whitened in blocks of `whiten_block` bins (0: not whitened).  complex128 [n_t/2]."""

@@ -89,3 +89,69 @@ def test_bad_arguments(oracle):
         oracle.blockmax(np.zeros((2, 4)), 0)
     with pytest.raises(ValueError):
         oracle.blockmax(np.zeros(4), 2)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# oracle.candidates (reading 20): pinned by a scan of the PLANE ITSELF that never forms block maxima
+# first, by counting identities, and by the C1 injected signal
+# ---------------------------------------------------------------------------------------------------------
+def _candidates_from_plane(p, blk, thr, cap):
+    """Independent route: walk the plane column by column; a column is a candidate iff it is >= thr (float32) and
+    no column of its block is larger and no earlier column of its block is equal."""
+    p32 = p.astype(np.float32)
+    thr = np.float32(thr)
+    out = []
+    for r in range(p.shape[0]):
+        for c in range(p.shape[1]):
+            b0, b1 = (c // blk) * blk, min((c // blk + 1) * blk, p.shape[1])
+            v = p32[r, c]
+            if v >= thr and all(p32[r, k] < v for k in range(b0, c)) and all(p32[r, k] <= v for k in range(c + 1, b1)):
+                out.append((r, c, float(v)))
+    return len(out), out[:cap]
+
+
+@pytest.mark.parametrize("rows,cols,blk,thr,cap", [(1, 7, 3, 1.0, 10), (3, 40, 8, 3.0, 100), (3, 40, 8, 3.0, 4),
+                                                   (4, 33, 5, 0.0, 1000), (2, 20, 4, 1e9, 5), (2, 20, 20, 2.0, 0)])
+def test_candidates_equal_plane_scan(oracle, rows, cols, blk, thr, cap):
+    rng = np.random.default_rng(rows + 10 * cols + blk)
+    p = rng.exponential(2.0, size=(rows, cols))
+    n, rr, cc, pp = oracle.candidates(p, blk, thr, cap)
+    n_ref, ref = _candidates_from_plane(p, blk, thr, cap)
+    assert n == n_ref
+    assert list(zip(rr.tolist(), cc.tolist(), pp.tolist())) == ref
+
+
+def test_candidates_counting_identities_and_order(oracle):
+    rng = np.random.default_rng(20)
+    p = rng.exponential(2.0, size=(6, 100))
+    n_blk = 13                                                    # ceil(100 / 8)
+    n0, r0, c0, p0 = oracle.candidates(p, 8, 0.0, 10 ** 6)        # threshold 0: every block of every row
+    assert n0 == 6 * n_blk == r0.size
+    assert oracle.candidates(p, 8, np.inf, 10)[0] == 0            # nothing is >= +inf
+    n1, r1, c1, p1 = oracle.candidates(p, 8, 5.0, 10 ** 6)
+    assert n1 == int((oracle.blockmax(p, 8)[0].astype(np.float32) >= np.float32(5.0)).sum())
+    assert np.all(p1.astype(np.float32) >= np.float32(5.0))
+    assert np.array_equal(p1, p[r1, c1].astype(np.float32))       # the reported power is the plane's float32 value there
+    key = r1 * 1000 + c1
+    assert np.all(np.diff(key) > 0)                               # ordered by (row, column), no duplicates
+    # the threshold is inclusive, in float32
+    v = float(np.float32(p1.min()))
+    assert oracle.candidates(p, 8, v, 10 ** 6)[0] == n1
+    assert oracle.candidates(p, 8, float(np.nextafter(np.float32(v), np.float32(np.inf))), 10 ** 6)[0] == n1 - 1
+    # truncation keeps a prefix and still counts everything
+    n2, r2, c2, p2 = oracle.candidates(p, 8, 5.0, 3)
+    assert n2 == n1 and np.array_equal(r2, r1[:3]) and np.array_equal(c2, c1[:3]) and np.array_equal(p2, p1[:3])
+
+
+def test_c1_signal_is_the_strongest_candidate(oracle):
+    """BASELINE.json configs[0]: the z = +20 signal at bin 20000 (peak power 39 against noise maxima of 20-27).  With
+    the threshold at 0.74 of the plane maximum the list holds only the signal's footprint -- its own row and the
+    neighbouring trials, all at the signal's bin -- and its strongest entry is (row of z = +20, column 20000)."""
+    wl = workload.make_config(1)
+    p = oracle.direct(wl.spectrum[0], wl.templates.astype(np.complex128))
+    n, rr, cc, pp = oracle.candidates(p, 384, 0.74 * p.max(), 1000)
+    assert 2 <= n <= 8 and n == rr.size
+    k = int(np.argmax(pp))
+    assert wl.z_values[rr[k]] == 20 and cc[k] == 20000
+    assert np.all(np.abs(cc - 20000) <= 4)
+    assert all(abs(wl.z_values[r] - 20) <= 6 for r in rr)
