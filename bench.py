@@ -368,13 +368,31 @@ def run_ours(args):
         d1.record(stream)
         barrier()
         te = max_over_ranks(d0.elapsed_time(d1), world, "cuda")
+        # down to the candidate list (reading 20): threshold at power 30 (templates of unit norm on unit-variance noise:
+        # mean power 2, so 30 is a 1e-6.5 tail per sample), capacity 4096 -> 64 KB come back instead of the 1.9 MB of maxima
+        cand_cap, cand_thr = 4096, 30.0
+        h_cand = torch.empty((cand_cap, 4), dtype=torch.int32).pin_memory()
+        h_cnt = torch.zeros((2,), dtype=torch.int32).pin_memory()
+        plan.detect_candidates_host(h_spec, cand_thr, cand_cap, h_cand, h_cnt, stream=stream)
+        barrier()
+        d0.record(stream)
+        for _ in range(det_steps):
+            plan.detect_candidates_host(h_spec, cand_thr, cand_cap, h_cand, h_cnt, stream=stream)
+        d1.record(stream)
+        barrier()
+        tc = max_over_ranks(d0.elapsed_time(d1), world, "cuda")
+        cand = {"what": "fdas_detect_candidates_host: block maxima >= threshold as an ordered (item, row, column, power) list",
+                "threshold": cand_thr, "capacity": cand_cap, "found": int(h_cnt[0]), "written": int(h_cnt[1]),
+                "e2e": {"value": whole_job_value(points, world, det_steps, tc), "unit": UNIT, "ms_per_step": tc / det_steps,
+                        "h2d_bytes_per_step": int(h_spec.numel() * 8), "d2h_bytes_per_step": 16 * cand_cap + 8, "steps": det_steps}}
         det_bytes = 8 * wl.n_batch * int(n_seg) * wl.seg_len + 8 * wl.n_z * wl.seg_len + 8 * wl.n_batch * wl.n_z * int(n_seg)
         detect = {"what": "fdas_detect_blockmax: same (z,r) points, per (row, segment) max + argmax instead of the plane",
                   "value": whole_job_value(points, world, args.steps, td), "unit": UNIT, "ms_per_step": td / args.steps,
                   "bytes_per_launch": det_bytes, "alu_frac": None,
                   "e2e": {"value": whole_job_value(points, world, det_steps, te), "unit": UNIT, "ms_per_step": te / det_steps,
                           "h2d_bytes_per_step": int(h_spec.numel() * 8), "d2h_bytes_per_step": int(h_max.numel() * 8),
-                          "steps": det_steps}}
+                          "steps": det_steps},
+                  "candidates": cand}
 
     if rank == 0:
         pk = peaks()

@@ -212,6 +212,35 @@ fdas_status fdas_detect_blockmax(fdas_plan *plan, const void *d_spectrum, float 
 fdas_status fdas_detect_blockmax_host(fdas_plan *plan, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream);
 
 /*
+ * Detection down to a candidate list ("detect", "FDAS code"; reading 20): fdas_detect_blockmax
+ * followed by a threshold on the block maxima.  A block maximum is a candidate iff its float32 power is >= threshold
+ * (inclusive); the list is ordered by (item, row, column), which makes it unique, and holds at most `capacity` entries:
+ *   d_cand        DEVICE, fdas_candidate [capacity], 4-byte aligned; entries [0, d_count[1]) are written, the rest is
+ *                 left untouched
+ *   d_count       DEVICE, int32 [2]: d_count[0] = number of candidates found (all of them, may exceed capacity: then
+ *                 the list holds the first `capacity` in order and d_count[0] - d_count[1] were dropped);
+ *                 d_count[1] = number written = min(found, capacity)
+ *   threshold     float32 power (templates of unit norm on whitened noise give a mean power of 2)
+ *   capacity      >= 0; n_batch * n_z * n_blk must be < 2^31
+ * The block maxima go to a plan-owned scratch buffer (8 bytes per (item, row, block) + 4 per row), allocated by the
+ * first call on the plan and when n_batch has grown since: that call allocates, later ones only launch (the hot kernel
+ * and three small ones).  Deterministic, no atomics.  One such call per plan at a time (they share the scratch).
+ * Otherwise as fdas_convolve (asynchronous, same errors, plus FDAS_ERR_ALLOC).  fdas_detect_candidates_host takes the
+ * spectrum from HOST memory and returns both results to HOST memory (h_cand [capacity], h_count [2]; 16 * capacity + 8
+ * bytes come back whatever the count, so entries of h_cand at and beyond h_count[1] are unspecified), uploads like fdas_detect_blockmax_host, and synchronises the stream.
+ */
+typedef struct {
+    int32_t item;    /* batch item */
+    int32_t row;     /* template row i <-> z = -z_max + i * z_step */
+    int32_t column;  /* r0 of the block maximum */
+    float power;     /* the float32 value the power plane would hold there */
+} fdas_candidate;
+fdas_status fdas_detect_candidates(fdas_plan *plan, const void *d_spectrum, float threshold, int capacity,
+                                   fdas_candidate *d_cand, int32_t *d_count, void *cuda_stream);
+fdas_status fdas_detect_candidates_host(fdas_plan *plan, const void *h_spectrum, float threshold, int capacity,
+                                        fdas_candidate *h_cand, int32_t *h_count, void *cuda_stream);
+
+/*
  * The segment FFT as a stand-alone batched transform (eq.(3); the stand-alone comparison of P:46 and
  * Table 1: "100 FFTs per kernel launch, while launching 1000 of these kernels", N = 1024, with the
  * number of elements per thread as the design axis).  Same device code as the convolution kernel's forward

@@ -30,6 +30,8 @@ SYMBOLS = {
     "fdas_convolve_complex": (_int, [_vp, _vp, _vp, _vp]),
     "fdas_detect_blockmax": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "fdas_detect_blockmax_host": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "fdas_detect_candidates": (_int, [_vp, _vp, ctypes.c_float, _int, _vp, _vp, _vp]),
+    "fdas_detect_candidates_host": (_int, [_vp, _vp, ctypes.c_float, _int, _vp, _vp, _vp]),
     "fdas_plan_destroy": (_int, [_vp]),
     "fdas_plan_nz": (_int, [_vp]),
     "fdas_plan_step": (_int, [_vp]),
@@ -54,6 +56,9 @@ SYMBOLS = {
     "fdas_debug_alu_peak": (_int, [_int, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
     "fdas_version": (ctypes.c_char_p, []),
 }
+
+# fdas_candidate (include/fdas.h): view a uint8 / int32 buffer of 16-byte records with this dtype
+CANDIDATE_DTYPE = np.dtype([("item", np.int32), ("row", np.int32), ("column", np.int32), ("power", np.float32)])
 
 _LIB = None
 
@@ -177,6 +182,15 @@ class Plan:
     def detect_blockmax_host(self, h_spectrum, h_max, h_arg, stream=None):
         _check(lib().fdas_detect_blockmax_host(self._h, _ptr(h_spectrum), _ptr(h_max), _ptr(h_arg), _stream(stream)),
                "fdas_detect_blockmax_host")
+
+    def detect_candidates(self, d_spectrum, threshold, capacity, d_cand, d_count, stream=None):
+        """d_cand: DEVICE [capacity] records of CANDIDATE_DTYPE (16 bytes); d_count: DEVICE int32 [2] = (found, written)."""
+        _check(lib().fdas_detect_candidates(self._h, _ptr(d_spectrum), float(threshold), int(capacity), _ptr(d_cand), _ptr(d_count),
+                                            _stream(stream)), "fdas_detect_candidates")
+
+    def detect_candidates_host(self, h_spectrum, threshold, capacity, h_cand, h_count, stream=None):
+        _check(lib().fdas_detect_candidates_host(self._h, _ptr(h_spectrum), float(threshold), int(capacity), _ptr(h_cand),
+                                                 _ptr(h_count), _stream(stream)), "fdas_detect_candidates_host")
 
     def destroy(self):
         if self._h:

@@ -23,6 +23,7 @@
 #include "convolve.cuh"
 #include "fft_batch.cuh"
 #include "spectrum.cuh"
+#include "detect.cuh"
 
 namespace fdas {
 
@@ -143,6 +144,8 @@ struct fdas_plan {
     float *d_host_power;
     void *d_host_det;
     size_t host_spec_bytes, host_power_bytes, host_det_bytes;
+    void *d_cand_scratch;                     // fdas_detect_candidates: block maxima, argmaxima, row offsets
+    size_t cand_scratch_bytes;
     cudaStream_t copy_stream;                 // fdas_detect_blockmax_host: chunked upload overlapping the kernel
     cudaEvent_t copy_event[HOST_CHUNKS + 1];
 };
@@ -648,25 +651,21 @@ fdas_status fdas_convolve_host(fdas_plan *p, const void *h_spectrum, float *h_po
     return FDAS_OK;
 }
 
-fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream)
+// Spectrum from HOST memory -> block maxima in DEVICE arrays d_max / d_arg, enqueued on the caller's stream (nothing
+// is downloaded, nothing synchronised): the common front of fdas_detect_blockmax_host and fdas_detect_candidates_host.
+// On an error it has drained what it had enqueued.
+static fdas_status blockmax_from_host(fdas_plan *p, const void *h_spectrum, float *d_max, int32_t *d_arg, void *cuda_stream)
 {
-    if (!p || !h_spectrum || !h_max || !h_arg) return FDAS_ERR_INVALID_ARG;
-    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
-    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
     const size_t sb = sizeof(float2) * (size_t)p->n_batch * (size_t)p->n_f;
-    const size_t nb = (size_t)p->n_batch * (size_t)p->n_z * (size_t)p->n_seg; // entries of each result array
     cudaError_t e = stage_reserve(&p->d_host_spec, &p->host_spec_bytes, sb);
-    if (e == cudaSuccess) e = stage_reserve(&p->d_host_det, &p->host_det_bytes, 8 * nb);
     if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
-    float *d_max = (float *)p->d_host_det;
-    int32_t *d_arg = (int32_t *)p->d_host_det + nb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     // The spectrum goes up in HOST_CHUNKS pieces on a plan-owned copy stream and every piece's segments are launched
     // as soon as it has arrived, so that all but the first piece of the host-to-device copy hides behind the kernel.
     // The pieces are ranges of work items = (batch item, segment) in order, i.e. contiguous ranges of the input.
     const int64_t n_work = p->n_seg * (int64_t)p->n_batch;
     // Every piece is about one full wave of the persistent grid or more: smaller launches would leave SMs idle.
-    // A call that is a single wave anyway goes the plain way: copy, launch and read back on the caller's stream.
+    // A call that is a single wave anyway goes the plain way: copy and launch on the caller's stream.
     const int64_t waves = (n_work + p->grid_max[OUT_BLOCKMAX] - 1) / p->grid_max[OUT_BLOCKMAX];
     const int n_chunks = (int)(waves > HOST_CHUNKS ? HOST_CHUNKS : waves);
     if (n_chunks <= 1) {
@@ -674,10 +673,6 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, floa
         if (e != cudaSuccess) return cuda_fail(p, e);
         fdas_status s1 = fdas_detect_blockmax(p, p->d_host_spec, d_max, d_arg, cuda_stream);
         if (s1 != FDAS_OK) { host_drain(p, st); return s1; }
-        e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
         return FDAS_OK;
     }
     e = ensure_copy_stream(p);
@@ -706,8 +701,99 @@ fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, floa
         if (s != FDAS_OK) { host_drain(p, st); return s; }
     }
     p->last_launches = n_chunks;
+    return FDAS_OK;
+}
+
+fdas_status fdas_detect_blockmax_host(fdas_plan *p, const void *h_spectrum, float *h_max, int32_t *h_arg, void *cuda_stream)
+{
+    if (!p || !h_spectrum || !h_max || !h_arg) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
+    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
+    const size_t nb = (size_t)p->n_batch * (size_t)p->n_z * (size_t)p->n_seg; // entries of each result array
+    cudaError_t e = stage_reserve(&p->d_host_det, &p->host_det_bytes, 8 * nb);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+    float *d_max = (float *)p->d_host_det;
+    int32_t *d_arg = (int32_t *)p->d_host_det + nb;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    fdas_status s = blockmax_from_host(p, h_spectrum, d_max, d_arg, cuda_stream);
+    if (s != FDAS_OK) return s;
     e = cudaMemcpyAsync(h_max, d_max, 4 * nb, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_arg, d_arg, 4 * nb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
+    return FDAS_OK;
+}
+
+// The plan-owned scratch of fdas_detect_candidates[_host]: [nb] float maxima | [nb] int32 offsets | [n_rows + 1] int32.
+struct CandScratch { float *d_max; int32_t *d_arg; int *d_rows; size_t nb; int n_rows; };
+
+static fdas_status cand_scratch(fdas_plan *p, int capacity, CandScratch *cs)
+{
+    const size_t nb = (size_t)p->n_batch * (size_t)p->n_z * (size_t)p->n_seg;
+    if (capacity < 0 || nb >= ((size_t)1 << 31)) return FDAS_ERR_INVALID_ARG;
+    const int n_rows = p->n_batch * p->n_z;
+    cudaError_t e = stage_reserve(&p->d_cand_scratch, &p->cand_scratch_bytes, 8 * nb + 4 * ((size_t)n_rows + 1));
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+    cs->d_max = (float *)p->d_cand_scratch;
+    cs->d_arg = (int32_t *)p->d_cand_scratch + nb;
+    cs->d_rows = (int *)p->d_cand_scratch + 2 * nb;
+    cs->nb = nb;
+    cs->n_rows = n_rows;
+    return FDAS_OK;
+}
+
+// block maxima (already enqueued on st) -> candidate list and counts, three small launches on st
+static cudaError_t cand_compact(fdas_plan *p, const CandScratch &cs, float threshold, int capacity, fdas_candidate *d_cand,
+                                int32_t *d_count, cudaStream_t st)
+{
+    const unsigned row_ctas = (unsigned)((cs.n_rows + 7) / 8); // 8 warps per CTA, one warp per (item, row)
+    fdas_cand_count_kernel<<<row_ctas, 256, 0, st>>>(cs.d_max, cs.n_rows, (long long)p->n_seg, threshold, cs.d_rows);
+    fdas_cand_scan_kernel<<<1, 1024, 0, st>>>(cs.d_rows, cs.n_rows, capacity, d_count);
+    fdas_cand_scatter_kernel<<<row_ctas, 256, 0, st>>>(cs.d_max, cs.d_arg, cs.n_rows, p->n_z, (long long)p->n_seg, p->S, threshold,
+                                                       cs.d_rows, capacity, d_cand);
+    p->last_launches += 3;
+    return cudaGetLastError();
+}
+
+fdas_status fdas_detect_candidates(fdas_plan *p, const void *d_spectrum, float threshold, int capacity, fdas_candidate *d_cand,
+                                   int32_t *d_count, void *cuda_stream)
+{
+    if (!p || !d_spectrum || !d_count || (!d_cand && capacity > 0)) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_spectrum & 7u) || ((uintptr_t)d_cand & 3u) || ((uintptr_t)d_count & 3u)) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
+    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
+    CandScratch cs;
+    fdas_status s = cand_scratch(p, capacity, &cs);
+    if (s != FDAS_OK) return s;
+    s = enqueue(p, OUT_BLOCKMAX, d_spectrum, nullptr, nullptr, cs.d_max, (int *)cs.d_arg, cuda_stream);
+    if (s != FDAS_OK) return s;
+    cudaError_t e = cand_compact(p, cs, threshold, capacity, d_cand, d_count, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return FDAS_OK;
+}
+
+fdas_status fdas_detect_candidates_host(fdas_plan *p, const void *h_spectrum, float threshold, int capacity, fdas_candidate *h_cand,
+                                        int32_t *h_count, void *cuda_stream)
+{
+    if (!p || !h_spectrum || !h_count || (!h_cand && capacity > 0)) return FDAS_ERR_INVALID_ARG;
+    if (!on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
+    if (!p->has_templates) return FDAS_ERR_NO_TEMPLATES;
+    CandScratch cs;
+    fdas_status s = cand_scratch(p, capacity, &cs);
+    if (s != FDAS_OK) return s;
+    // the device copies of the two results: 16 * capacity + 8 bytes behind the spectrum's staging-independent buffer
+    const size_t out_bytes = sizeof(fdas_candidate) * (size_t)capacity + 8;
+    cudaError_t e = stage_reserve(&p->d_host_det, &p->host_det_bytes, out_bytes);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p->last_cuda_error = (int)e; return FDAS_ERR_ALLOC; }
+    int32_t *d_count = (int32_t *)p->d_host_det;
+    fdas_candidate *d_cand = (fdas_candidate *)((unsigned char *)p->d_host_det + 8);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s = blockmax_from_host(p, h_spectrum, cs.d_max, cs.d_arg, cuda_stream);
+    if (s != FDAS_OK) return s;
+    e = cand_compact(p, cs, threshold, capacity, d_cand, d_count, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_count, d_count, 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && capacity > 0)
+        e = cudaMemcpyAsync(h_cand, d_cand, sizeof(fdas_candidate) * (size_t)capacity, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { host_drain(p, st); return cuda_fail(p, e); }
     return FDAS_OK;
@@ -722,6 +808,7 @@ fdas_status fdas_plan_destroy(fdas_plan *p)
     if (p->d_host_spec) cudaFree(p->d_host_spec);
     if (p->d_host_power) cudaFree(p->d_host_power);
     if (p->d_host_det) cudaFree(p->d_host_det);
+    if (p->d_cand_scratch) cudaFree(p->d_cand_scratch);
     if (p->copy_stream) {
         for (int i = 0; i <= HOST_CHUNKS; ++i) if (p->copy_event[i]) cudaEventDestroy(p->copy_event[i]);
         cudaStreamDestroy(p->copy_stream);

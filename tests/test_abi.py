@@ -84,6 +84,9 @@ def test_round2_entries_validate_before_touching_the_gpu():
     assert L.fdas_detect_blockmax(None, None, None, None, None) == B.FDAS_ERR_INVALID_ARG
     assert L.fdas_detect_blockmax_host(None, None, None, None, None) == B.FDAS_ERR_INVALID_ARG
     assert L.fdas_plan_set_symmetry(None, 1) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_detect_candidates(None, None, 1.0, 8, None, None, None) == B.FDAS_ERR_INVALID_ARG
+    assert L.fdas_detect_candidates_host(None, None, 1.0, 8, None, None, None) == B.FDAS_ERR_INVALID_ARG
+    assert B.CANDIDATE_DTYPE.itemsize == 16
     assert L.fdas_plan_symmetry_active(None) == 0 and L.fdas_plan_grid(None) == 0
     out = ctypes.c_void_p()
     # stand-alone FFT: (n, elements per thread) combinations that do not exist
