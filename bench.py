@@ -75,7 +75,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the plane the oracle is timed on (0 = auto)")
-    ap.add_argument("--mode", default="convolve", choices=["convolve", "fft", "peak", "general"],
+    ap.add_argument("--mode", default="convolve", choices=["convolve", "fft", "peak", "general", "spectrum"],
                     help="convolve: the FDAS hot path (BASELINE.json metric); fft: the stand-alone FFT protocol of Table 1")
     ap.add_argument("--fft-n", type=int, default=1024)
     ap.add_argument("--no-detect", action="store_true", help="skip the fused block-maximum (detection) timings")
@@ -563,6 +563,56 @@ def run_general(args):
     return 0
 
 
+def run_spectrum(args):
+    """--mode spectrum: the step before the correlation (fdas_spectrum_exec, reading 18) on the 2^23-sample
+    series behind BASELINE.json config 3: real series -> 2^22 whitened bins.  HBM-bound by construction: the algorithmic
+    traffic is 4 bytes per sample in and 8 bytes per bin out; every extra pass over the data shows in the fraction."""
+    import torch
+    from paper_1711_10855_b200 import binding
+    binding.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    n_t, blk = 1 << 23, 4096
+    g = torch.Generator(device="cuda").manual_seed(171110855)
+    n_rot = 8                                                     # 8 x 33.5 MB of input > L2
+    xs = [torch.randn(n_t, device="cuda", generator=g) for _ in range(n_rot)]
+    out = torch.empty(n_t // 2, dtype=torch.complex64, device="cuda")
+    plan = binding.SpectrumPlan(n_t, blk)
+    stream = torch.cuda.Stream()
+    pk = peaks()
+    for i in range(max(3, args.warmup)):
+        plan.exec(xs[i % n_rot], out, stream=stream)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.25)
+    t0 = time.time()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record(stream)
+    for i in range(args.steps):
+        plan.exec(xs[i % n_rot], out, stream=stream)
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop(t0, time.time())
+    per = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    ms = ev[0].elapsed_time(ev[-1]) / args.steps
+    byt = 4 * n_t + 8 * (n_t // 2)
+    gbs = byt / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "spectrum_bins_per_s", "value": (n_t // 2) / (ms * 1e-3), "unit": "bins/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "ms_median": float(np.median(per)),
+                      "ms_min": float(np.min(per)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f32", "data": "synthetic", "gpu_launches": 6 * args.steps,
+                      "config": {"workload": f"real series of {n_t} float32 samples -> {n_t // 2} whitened complex64 bins (whiten_block {blk})",
+                                 "l2": f"inputs rotate over {n_rot} series ({n_rot * 4 * n_t / 1e6:.0f} MB) > 126 MB L2"},
+                      "clocks": clocks,
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gbs / pk["hbm_gbs"],
+                                   "traffic": None, "bytes_per_launch": byt,
+                                   "note": "bytes_per_launch is per fdas_spectrum_exec (six kernel launches): samples in + bins out"},
+                      "kernel_version": binding.version()}))
+    plan.destroy()
+    return 0
+
+
 def run_peak(args):
     """--mode peak: the FP32 FMA rate of this GPU on register-only chains (fdas_debug_alu_peak) next to the nominal
     figure the "alu" roofline uses, with the clocks seen meanwhile."""
@@ -645,6 +695,8 @@ def main():
         return run_peak(args)
     if args.mode == "general":
         return run_general(args)
+    if args.mode == "spectrum":
+        return run_spectrum(args)
     return run_ours(args)
 
 

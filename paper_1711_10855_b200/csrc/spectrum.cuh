@@ -13,6 +13,26 @@
 
 namespace fdas {
 
+// exp(i pi scale e / n) for 0 <= e < n, n a power of two, scale = -1 or -2, as float2 (cos, sin).
+// For n <= 2^24 the fraction e / n is exact in float32 (e has at most 24 bits, n is a power of two) and sincospif
+// reduces its argument exactly, so the result is within 1 ulp of the true root -- what rounding a double evaluation
+// would give to half an ulp -- at a small fraction of its cost (the double version was 15 us of the 25 us of the
+// twiddling transpose and 20 us of the 34 us of the last pass at n = 2^22; profiles/r3_spectrum.md).
+// Longer transforms keep the double evaluation: there e / n does not fit a float.
+__device__ __forceinline__ float2 unit_root(long long e, long long n, float scale)
+{
+    float s, c;
+    if (n <= (1ll << 24)) {
+        sincospif(scale * ((float)e * (1.0f / (float)n)), &s, &c);
+    } else {
+        double sd, cd;
+        sincospi((double)scale * (double)e / (double)n, &sd, &cd);
+        s = (float)sd;
+        c = (float)cd;
+    }
+    return make_float2(c, s);
+}
+
 // out[c][r] = in[r][c] (* w_N^{r c} if TWIDDLE), in: [rows][cols] complex64.  32 x 32 tiles through shared memory,
 // 32 x 8 threads; rows and cols are multiples of 32.
 template <bool TWIDDLE>
@@ -27,12 +47,10 @@ __global__ void __launch_bounds__(256) fdas_transpose_kernel(const float2 *__res
         const int r = r0 + ty + j, c = c0 + tx;
         float2 v = __ldcs(in + (size_t)r * cols + c);
         if (TWIDDLE) {
-            // w_N^{r c} = exp(-2 pi i (r c mod N) / N); r c < 2^26, the angle is formed in double and rounded once
-            const long long e = ((long long)r * c) % n_total;
-            double s, co;
-            sincospi(-2.0 * (double)e / (double)n_total, &s, &co);
-            const float wr = (float)co, wi = (float)s;
-            v = make_float2(v.x * wr - v.y * wi, v.x * wi + v.y * wr);
+            // w_N^{r c} = exp(-2 pi i (r c mod N) / N)
+            const long long e = ((long long)r * c) & (n_total - 1); // N is a power of two
+            const float2 w = unit_root(e, n_total, -2.0f);
+            v = make_float2(v.x * w.x - v.y * w.y, v.x * w.y + v.y * w.x);
         }
         tile[ty + j][tx] = v;
     }
@@ -57,19 +75,40 @@ __global__ void __launch_bounds__(256) fdas_rfft_whiten_kernel(const float2 *__r
     const long long b1 = b0 + width < N ? b0 + width : N;
     __shared__ float red[8];
     __shared__ float s_scale;
-    float acc = 0.f;
-    for (long long k = b0 + threadIdx.x; k < b1; k += blockDim.x) {
+    // bin k of the real series' transform from Z_k and Z_{N-k}
+    auto bin = [&](long long k) {
         const float2 zk = __ldg(Z + k);
         const float2 zc = __ldg(Z + ((N - k) & (N - 1)));       // conj applied below
         const float er = 0.5f * (zk.x + zc.x), ei = 0.5f * (zk.y - zc.y);
         const float orr = 0.5f * (zk.y + zc.y), oi = -0.5f * (zk.x - zc.x);
-        double s, c;
-        sincospi(-(double)k / (double)N, &s, &c);               // w_{2N}^k = exp(-i pi k / N)
-        const float wr = (float)c, wi = (float)s;
-        float2 x = make_float2(er + (orr * wr - oi * wi), ei + (orr * wi + oi * wr));
+        const float2 w = unit_root(k, N, -1.0f);                 // w_{2N}^k = exp(-i pi k / N)
+        float2 x = make_float2(er + (orr * w.x - oi * w.y), ei + (orr * w.y + oi * w.x));
         if (whiten && k == 0) x = make_float2(0.f, 0.f);
-        acc += x.x * x.x + x.y * x.y;
-        out[k] = x;
+        return x;
+    };
+    // Blocks of up to 16 bins per thread (blk <= 4096, the usual case) stay in registers between the two phases, so the
+    // spectrum is written once; wider blocks are written unscaled and rescaled in place (each thread its own bins).
+    constexpr int PER = 16;
+    const bool in_regs = width <= (long long)PER * blockDim.x;
+    float2 xr[PER];
+    float acc = 0.f;
+    if (in_regs) {
+#pragma unroll
+        for (int i = 0; i < PER; ++i) {
+            const long long k = b0 + threadIdx.x + (long long)i * blockDim.x;
+            xr[i] = make_float2(0.f, 0.f);
+            if (k < b1) {
+                xr[i] = bin(k);
+                acc += xr[i].x * xr[i].x + xr[i].y * xr[i].y;
+                if (!whiten) out[k] = xr[i];
+            }
+        }
+    } else {
+        for (long long k = b0 + threadIdx.x; k < b1; k += blockDim.x) {
+            const float2 x = bin(k);
+            acc += x.x * x.x + x.y * x.y;
+            out[k] = x;
+        }
     }
     if (!whiten) return;
 #pragma unroll
@@ -84,9 +123,17 @@ __global__ void __launch_bounds__(256) fdas_rfft_whiten_kernel(const float2 *__r
     }
     __syncthreads();
     const float sc = s_scale;
-    for (long long k = b0 + threadIdx.x; k < b1; k += blockDim.x) { // each thread rescales what it wrote itself
-        const float2 x = out[k];
-        out[k] = make_float2(x.x * sc, x.y * sc);
+    if (in_regs) {
+#pragma unroll
+        for (int i = 0; i < PER; ++i) {
+            const long long k = b0 + threadIdx.x + (long long)i * blockDim.x;
+            if (k < b1) __stcs(out + k, make_float2(xr[i].x * sc, xr[i].y * sc));
+        }
+    } else {
+        for (long long k = b0 + threadIdx.x; k < b1; k += blockDim.x) { // each thread rescales what it wrote itself
+            const float2 x = out[k];
+            out[k] = make_float2(x.x * sc, x.y * sc);
+        }
     }
 }
 
