@@ -508,6 +508,7 @@ def run_fft(args):
                       "l2": f"input and output {n_total * n * 8 / 1e9:.2f} GB each >> 126 MB L2"},
            "variants": rows, "clocks": clocks, "gpu_launches": launches,
            "paper_context": "Table 1 (P:56-60): 1.80 ms on P100, 2.21 ms on TITAN X (Pascal) for 100 000 FFTs, N = 1024; other hardware, not a target",
+           "protocol_note": "protocol_1000x100_ms: fdas_fft_exec_many = 1000 launches of 100 transforms each over 100 000 distinct sequences, recorded once as a four-chain CUDA graph and launched per repetition",
            "roofline": {"bound": "hbm", "achieved": best["hbm_gbs"], "peak": pk["hbm_gbs"], "unit": "GB/s",
                         "frac": best["hbm_frac"], "traffic": ncu_traffic(f"fft{n}e{best['elems_per_thread']}", binding.version())[0],
                         "kernel": "fdas::fdas_fft_batch_kernel",

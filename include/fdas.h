@@ -259,7 +259,11 @@ fdas_status fdas_fft_exec(fdas_fft_plan *plan, int64_t n_fft, const void *d_in, 
 /* The repetition scheme of P:46: n_launches launches of n_fft transforms each, enqueued back to back.  Launch i
  * transforms sequences [i*n_fft, (i+1)*n_fft), so d_in and d_out are DEVICE complex64 [n_launches * n_fft][n] and the
  * 1000 x 100 protocol reads and writes 100 000 distinct sequences (from and to HBM), the same data as one launch of
- * 100 000. */
+ * 100 000.  From 8 launches on, the launches are recorded once as a CUDA graph (the same kernels; as they touch
+ * disjoint sequences the graph orders launch i only after launch i-4, four chains that may overlap on the GPU) and
+ * the graph is launched on cuda_stream, in order with the stream's other work: the first call with a given argument set
+ * does that host-side work (milliseconds) and allocates the graph; calls repeating the last argument set only launch it.
+ * One call per plan at a time. */
 fdas_status fdas_fft_exec_many(fdas_fft_plan *plan, int n_launches, int64_t n_fft, const void *d_in, void *d_out,
                                int inverse, void *cuda_stream);
 fdas_status fdas_fft_plan_destroy(fdas_fft_plan *plan);

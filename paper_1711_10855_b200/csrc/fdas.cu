@@ -351,6 +351,15 @@ template <bool PACKED> __global__ void __launch_bounds__(512) fdas_alu_peak_kern
 struct fdas_fft_plan {
     int n, e, device, grid_max;
     float2 *d_tw;
+    // fdas_fft_exec_many: the last protocol (argument set) as an instantiated CUDA graph, and the stream it was captured on
+    cudaGraphExec_t many_exec;
+    cudaStream_t many_stream;
+    cudaStream_t many_side[3];   // capture-time side branches (MANY_BRANCHES - 1)
+    cudaEvent_t many_fork, many_join[3];
+    int many_launches, many_inverse;
+    int64_t many_n_fft;
+    const void *many_in;
+    void *many_out;
 };
 
 template <class C> static cudaError_t fft_batch_prepare(int device, int *grid_max)
@@ -863,11 +872,10 @@ fdas_status fdas_fft_exec(fdas_fft_plan *p, int64_t n_fft, const void *d_in, voi
     return FDAS_OK;
 }
 
-fdas_status fdas_fft_exec_many(fdas_fft_plan *p, int n_launches, int64_t n_fft, const void *d_in, void *d_out, int inverse,
-                               void *cuda_stream)
+// launch i transforms sequences [i * n_fft, (i+1) * n_fft): 1000 x 100 walks 100 000 distinct sequences through HBM
+static fdas_status fft_exec_loop(fdas_fft_plan *p, int n_launches, int64_t n_fft, const void *d_in, void *d_out, int inverse,
+                                 void *cuda_stream)
 {
-    if (!p || n_launches < 0 || n_fft < 0) return FDAS_ERR_INVALID_ARG;
-    // launch i transforms sequences [i * n_fft, (i+1) * n_fft): 1000 x 100 walks 100 000 distinct sequences through HBM
     const size_t stride = (size_t)n_fft * (size_t)p->n;   // complex64 elements per launch
     for (int i = 0; i < n_launches; ++i) {
         fdas_status s = fdas_fft_exec(p, n_fft, (const float2 *)d_in + i * stride, (float2 *)d_out + i * stride, inverse, cuda_stream);
@@ -876,9 +884,81 @@ fdas_status fdas_fft_exec_many(fdas_fft_plan *p, int n_launches, int64_t n_fft, 
     return FDAS_OK;
 }
 
+fdas_status fdas_fft_exec_many(fdas_fft_plan *p, int n_launches, int64_t n_fft, const void *d_in, void *d_out, int inverse,
+                               void *cuda_stream)
+{
+    if (!p || !d_in || !d_out || n_launches < 0 || n_fft < 0 || d_in == d_out) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in & 7u) || ((uintptr_t)d_out & 7u)) return FDAS_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return FDAS_ERR_INVALID_ARG;
+    if (n_launches == 0 || n_fft == 0) return FDAS_OK;
+    // A handful of launches go out one by one.  A long protocol is launch-rate bound that way (1000 launches cost 4.1 ms
+    // of host-side launch intervals for 0.3 ms of work, profiles/r2_side_benchmarks.md), so it is recorded once as a CUDA
+    // graph of the same n_launches kernels and the graph is launched; it is kept for the next call with the same
+    // arguments.  The launches touch disjoint sequences, so nothing orders them but the stream they used to share: the
+    // graph says so, as MANY_BRANCHES chains (launch i follows launch i - MANY_BRANCHES), which lets the GPU start a
+    // launch while its neighbours run (one chain: 2.65 ms for 1000 x 100, a dependent launch every 2.6 us).
+    constexpr int GRAPH_FROM = 8, MANY_BRANCHES = 4;
+    if (n_launches < GRAPH_FROM) return fft_exec_loop(p, n_launches, n_fft, d_in, d_out, inverse, cuda_stream);
+    inverse = inverse != 0;
+    const bool hit = p->many_exec && p->many_launches == n_launches && p->many_n_fft == n_fft && p->many_in == d_in &&
+                     p->many_out == d_out && p->many_inverse == inverse;
+    if (!hit) {
+        if (p->many_exec) { cudaGraphExecDestroy(p->many_exec); p->many_exec = nullptr; }
+        cudaError_t e = cudaSuccess;
+        if (!p->many_stream) {
+            e = cudaStreamCreateWithFlags(&p->many_stream, cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->many_fork, cudaEventDisableTiming);
+            for (int b = 0; b < MANY_BRANCHES - 1 && e == cudaSuccess; ++b) {
+                e = cudaStreamCreateWithFlags(&p->many_side[b], cudaStreamNonBlocking);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->many_join[b], cudaEventDisableTiming);
+            }
+        }
+        if (e == cudaSuccess) e = cudaStreamBeginCapture(p->many_stream, cudaStreamCaptureModeThreadLocal);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+        // fork the side branches off the capturing stream, deal the launches round robin, join them again
+        e = cudaEventRecord(p->many_fork, p->many_stream);
+        for (int b = 0; b < MANY_BRANCHES - 1 && e == cudaSuccess; ++b) e = cudaStreamWaitEvent(p->many_side[b], p->many_fork, 0);
+        fdas_status s = e == cudaSuccess ? FDAS_OK : FDAS_ERR_CUDA;
+        const size_t stride = (size_t)n_fft * (size_t)p->n;
+        for (int i = 0; i < n_launches && s == FDAS_OK; ++i) {
+            cudaStream_t bs = (i % MANY_BRANCHES) ? p->many_side[i % MANY_BRANCHES - 1] : p->many_stream;
+            s = fdas_fft_exec(p, n_fft, (const float2 *)d_in + i * stride, (float2 *)d_out + i * stride, inverse, (void *)bs);
+        }
+        for (int b = 0; b < MANY_BRANCHES - 1 && s == FDAS_OK; ++b) {
+            e = cudaEventRecord(p->many_join[b], p->many_side[b]);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(p->many_stream, p->many_join[b], 0);
+            if (e != cudaSuccess) s = FDAS_ERR_CUDA;
+        }
+        cudaGraph_t graph = nullptr;
+        e = cudaStreamEndCapture(p->many_stream, &graph);   // also ends a capture that a failed launch invalidated
+        if (s == FDAS_OK && e == cudaSuccess) e = cudaGraphInstantiate(&p->many_exec, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+        if (s != FDAS_OK || e != cudaSuccess) {
+            (void)cudaGetLastError();
+            p->many_exec = nullptr;
+            return s != FDAS_OK ? s : FDAS_ERR_CUDA;
+        }
+        p->many_launches = n_launches;
+        p->many_n_fft = n_fft;
+        p->many_in = d_in;
+        p->many_out = d_out;
+        p->many_inverse = inverse;
+    }
+    if (cudaGraphLaunch(p->many_exec, (cudaStream_t)cuda_stream) != cudaSuccess) { (void)cudaGetLastError(); return FDAS_ERR_CUDA; }
+    return FDAS_OK;
+}
+
 fdas_status fdas_fft_plan_destroy(fdas_fft_plan *p)
 {
     if (!p) return FDAS_OK;
+    if (p->many_exec) cudaGraphExecDestroy(p->many_exec);
+    if (p->many_stream) cudaStreamDestroy(p->many_stream);
+    if (p->many_fork) cudaEventDestroy(p->many_fork);
+    for (int b = 0; b < 3; ++b) {
+        if (p->many_side[b]) cudaStreamDestroy(p->many_side[b]);
+        if (p->many_join[b]) cudaEventDestroy(p->many_join[b]);
+    }
     if (p->d_tw) cudaFree(p->d_tw);
     (void)cudaGetLastError();
     free(p);

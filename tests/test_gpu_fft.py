@@ -84,20 +84,38 @@ def test_batched_fft_arguments():
     plan.destroy()
 
 
-def test_exec_many_walks_the_buffers():
+@pytest.mark.parametrize("n_launches,per", [(7, 13), (40, 5)])
+def test_exec_many_walks_the_buffers(n_launches, per):
     """fdas_fft_exec_many ("100 FFTs per kernel launch, while launching 1000 of these kernels"): launch i
-    transforms sequences [i*n_fft, (i+1)*n_fft), so the protocol equals one launch over all of them, bit for bit."""
+    transforms sequences [i*n_fft, (i+1)*n_fft), so the protocol equals one launch over all of them, bit for bit --
+    as a loop of launches (7 launches) and as the recorded CUDA graph (40 launches: first call builds it, the second
+    re-uses it, other arguments rebuild it)."""
     import torch
     from paper_1711_10855_b200 import binding
-    n, n_launches, per = 1024, 7, 13
+    n = 1024
     g = torch.Generator(device="cuda").manual_seed(46)
     x = torch.randn((n_launches * per, n, 2), device="cuda", generator=g)
     plan = binding.FftPlan(n)
     y_one = torch.full_like(x, float("nan"))
-    y_many = torch.full_like(x, float("nan"))
     plan.exec(n_launches * per, x, y_one)
-    plan.exec_many(n_launches, per, x, y_many)
+    stream = torch.cuda.Stream()
     torch.cuda.synchronize()
-    assert torch.isfinite(y_many).all()
-    assert torch.equal(y_one, y_many)
+    for rep in range(3):
+        y_many = torch.full_like(x, float("nan"))
+        if rep < 2:
+            y_keep = y_many if rep == 0 else y_keep
+            target = y_keep                      # same arguments twice: the second call launches the cached graph
+            target.fill_(float("nan"))
+        else:
+            target = y_many                      # another output buffer: the graph is rebuilt
+        torch.cuda.synchronize()
+        plan.exec_many(n_launches, per, x, target, stream=stream)
+        torch.cuda.synchronize()
+        assert torch.isfinite(target).all()
+        assert torch.equal(y_one, target), rep
+    # the inverse through the same entry, and back
+    y_inv = torch.empty_like(x)
+    plan.exec_many(n_launches, per, y_one, y_inv, inverse=True, stream=stream)
+    torch.cuda.synchronize()
+    assert (y_inv / n - x).abs().max().item() < 2e-5
     plan.destroy()
