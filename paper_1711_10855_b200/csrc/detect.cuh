@@ -22,7 +22,13 @@ __global__ void __launch_bounds__(256) fdas_cand_count_kernel(const float *__res
     if (w >= n_rows) return;
     const float *b = bmax + (long long)w * n_blk;
     int c = 0;
-    for (long long s = lane; s < n_blk; s += 32) c += (b[s] >= thr) ? 1 : 0;
+    for (long long s0 = lane; s0 < n_blk; s0 += 128) { // four independent loads in flight per lane
+        float v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = (s0 + 32 * u < n_blk) ? b[s0 + 32 * u] : -1.f;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) c += (s0 + 32 * u < n_blk && v[u] >= thr) ? 1 : 0;
+    }
     c = __reduce_add_sync(0xffffffffu, c);
     if (lane == 0) row_count[w] = c;
 }
@@ -72,21 +78,30 @@ __global__ void __launch_bounds__(256) fdas_cand_scatter_kernel(const float *__r
     if (base >= capacity) return; // the list is already full before this row
     const float *b = bmax + (long long)w * n_blk;
     const int *a = barg + (long long)w * n_blk;
-    for (long long s0 = 0; s0 < n_blk && base < capacity; s0 += 32) {
-        const long long s = s0 + lane;
-        const float v = s < n_blk ? b[s] : 0.f;
-        const bool hit = s < n_blk && v >= thr;
-        const unsigned m = __ballot_sync(0xffffffffu, hit);
-        const int pos = base + __popc(m & ((1u << lane) - 1u));
-        if (hit && pos < capacity) {
-            fdas_candidate c;
-            c.item = w / n_z;
-            c.row = w % n_z;
-            c.column = (int32_t)(s * blk + a[s]);
-            c.power = v;
-            cand[pos] = c;
+    const int row_end = row_offset[w + 1];   // one past this row's last place: nothing left to find beyond it
+    for (long long s0 = 0; s0 < n_blk && base < capacity && base < row_end; s0 += 128) {
+        float v[4];                           // four independent loads in flight per lane, consumed in column order
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const long long s = s0 + 32 * u + lane;
+            v[u] = s < n_blk ? b[s] : 0.f;
         }
-        base += __popc(m);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const long long s = s0 + 32 * u + lane;
+            const bool hit = s < n_blk && v[u] >= thr;
+            const unsigned m = __ballot_sync(0xffffffffu, hit);
+            const int pos = base + __popc(m & ((1u << lane) - 1u));
+            if (hit && pos < capacity) {
+                fdas_candidate c;
+                c.item = w / n_z;
+                c.row = w % n_z;
+                c.column = (int32_t)(s * blk + a[s]);
+                c.power = v[u];
+                cand[pos] = c;
+            }
+            base += __popc(m);
+        }
     }
 }
 
